@@ -1,0 +1,217 @@
+"""P2 / P5 / P7 / P8 -- oracle push, deposit, boundary and sort against closed forms, invariants
+and brute force.  PAPER.md L35, L41, L63-67, L128-138, L150-156, L160-192."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from helpers import params, load
+
+
+def _one_species(Nc, kappa, bc=0, cap=4096, inv_ratio=1.0, **kw):
+    p = params(0, n_cells=Nc, ppc=1, mcc=False, n_species=1, bc=bc, **kw)
+    p["species"][0].update(kappa=kappa, capacity=cap)
+    p["sort_inv_ratio"] = inv_ratio
+    return p
+
+
+# ---- P5 push ---------------------------------------------------------------------------------
+def test_push_constant_field_closed_form():
+    Nc, kappa, E0 = 64, -0.25, 0.125          # all dyadic: the closed form is exact in fp32
+    o = O.Oracle(_one_species(Nc, kappa))
+    x0 = np.array([10.5, 30.25, 50.0], np.float32)
+    v0 = np.array([0.5, -0.25, 0.0], np.float32)
+    z = np.zeros(3, np.float32)
+    load(o, [(x0, v0, z + 1, z + 2)])
+    for n in range(1, 9):
+        o.set_E32(np.full(Nc + 1, E0, np.float32))
+        o.step(1)
+        assert np.array_equal(o.debug_get(O.VX), v0 + n * kappa * E0)
+        xs = np.sort(x0 + n * v0 + kappa * E0 * n * (n + 1) / 2)
+        assert np.array_equal(np.sort(o.debug_get(O.X)), xs.astype(np.float32))
+        assert np.array_equal(np.sort(o.debug_get(O.VY)), z + 1)      # vy, vz untouched
+        assert np.array_equal(np.sort(o.debug_get(O.VZ)), z + 2)
+
+
+def test_push_linear_field_leapfrog_oscillator():
+    # E = alpha (x - c): x_{n+1} - 2 x_n + x_{n-1} = kappa alpha (x_n - c); cos(w dt) = 1 + kappa alpha / 2
+    Nc, kappa, alpha, c = 128, -1.0, 0.01, 64.0
+    o = O.Oracle(_one_species(Nc, kappa))
+    E = (alpha * (np.arange(Nc + 1) - c)).astype(np.float32)
+    load(o, [(np.array([70.3], np.float32), np.zeros(1, np.float32), np.zeros(1, np.float32),
+              np.zeros(1, np.float32))])
+    xs = [70.3]
+    for n in range(200):
+        o.set_E32(E)
+        o.step(1)
+        xs.append(float(o.debug_get(O.X)[0]))
+    xs = np.array(xs)
+    res = xs[2:] - 2 * xs[1:-1] + xs[:-2] - kappa * alpha * (xs[1:-1] - c)
+    assert np.max(np.abs(res)) < 3e-5                      # fp32 rounding at x ~ 64
+    d = xs - c
+    zc = np.nonzero((d[:-1] > 0) & (d[1:] <= 0))[0]
+    tz = zc + d[zc] / (d[zc] - d[zc + 1])
+    w = 2 * np.pi / np.mean(np.diff(tz))
+    assert abs(w - np.arccos(1 + kappa * alpha / 2)) < 2e-4
+
+
+def test_gather_is_linear_interpolation():
+    Nc = 16
+    o = O.Oracle(_one_species(Nc, 1.0))
+    E = np.arange(Nc + 1, dtype=np.float32) ** 2
+    x0 = np.array([3.25, 7.5, 0.0, 15.75], np.float32)
+    z = np.zeros(4, np.float32)
+    load(o, [(x0, z, z, z)])
+    o.set_E32(E * np.float32(2.0 ** -10))
+    o.step(1)
+    j = np.floor(x0)
+    f = x0 - j
+    want = ((1 - f) * j ** 2 + f * (j + 1) ** 2) * 2.0 ** -10
+    assert np.allclose(np.sort(o.debug_get(O.VX)), np.sort(want), rtol=1e-6)
+
+
+# ---- P2 deposit ------------------------------------------------------------------------------
+def test_deposit_single_particle_and_sum():
+    Nc = 32
+    p = params(0, n_cells=Nc, ppc=1, mcc=False)
+    o = O.Oracle(p)
+    z1 = np.zeros(1, np.float32)
+    load(o, [(np.array([5.25], np.float32), z1, z1, z1), (np.array([31.75], np.float32), z1, z1, z1)])
+    rho, _, _ = o.get_rho_phi_E()
+    want = np.zeros(Nc + 1)
+    want[5], want[6] = -0.75, -0.25          # electron: sign -1
+    want[31], want[32] = 0.25, 0.75          # ion at the last cell touches the wall node
+    assert np.array_equal(rho, want)
+    assert np.array_equal(o.moments(0)["density"], -np.minimum(want, 0))
+
+
+def test_deposit_exact_total_and_bruteforce_hat():
+    Nc, n = 24, 5000
+    rng = np.random.default_rng(3)
+    p = params(0, n_cells=Nc, ppc=1, mcc=False, capacity_factor=300)
+    o = O.Oracle(p)
+    xe = np.minimum(rng.random(n, dtype=np.float32) * Nc, np.nextafter(np.float32(Nc), np.float32(0)))
+    xi = np.minimum(rng.random(n // 2, dtype=np.float32) * Nc, np.float32(Nc - 0.001))
+    load(o, [(xe, 0 * xe, 0 * xe, 0 * xe), (xi, 0 * xi, 0 * xi, 0 * xi)])
+    de, di = o.moments(0)["density"], o.moments(1)["density"]
+    assert de.sum() == n and di.sum() == n // 2           # exact: weights are dyadic
+    nodes = np.arange(Nc + 1)[:, None]
+    hat = lambda x: np.maximum(0.0, 1.0 - np.abs(x.astype(np.float64)[None, :] - nodes)).sum(1)
+    assert np.allclose(de, hat(xe), atol=1e-9) and np.allclose(di, hat(xi), atol=1e-9)
+    rho, _, _ = o.get_rho_phi_E()
+    assert np.allclose(rho, di - de, atol=1e-12)
+
+
+def test_deposit_periodic_wrap_and_background():
+    Nc = 8
+    p = params(1, n_cells=Nc, ppc=1)
+    o = O.Oracle(p)
+    x = np.array([7.5, 0.25], np.float32)
+    load(o, [(x, 0 * x, 0 * x, 0 * x)])
+    rho, _, _ = o.get_rho_phi_E()
+    want = np.full(Nc, p["background_rho"])
+    want[7] -= 0.5
+    want[0] -= 0.5 + 0.75
+    want[1] -= 0.25
+    assert np.allclose(rho, want, atol=1e-15)
+
+
+# ---- P7 boundary ----------------------------------------------------------------------------
+def test_absorption_bookkeeping_order_and_ties():
+    Nc = 16
+    o = O.Oracle(_one_species(Nc, 0.0))
+    x0 = np.array([0.5, 15.5, 8.0, 0.25, 15.0, 3.0, 1.0], np.float32)
+    v0 = np.array([-1.0, 1.0, 0.5, -0.25, 1.0, -3.0, 0.0], np.float32)   # x' = -.5, 16.5, 8.5, 0, 16, 0, 1
+    tag = np.arange(7, dtype=np.float32)
+    load(o, [(x0, v0, tag, tag)])
+    # the load sorted the particles; remember which tag sits where, then step
+    o.set_E32(np.zeros(Nc + 1, np.float32))
+    o.step(1)
+    m = o.moments(0)
+    assert (m["absorbed_left"], m["absorbed_right"], m["count"]) == (1, 2, 4)   # x'=16 exactly is absorbed
+    xs, tg = o.debug_get(O.X), o.debug_get(O.VY)
+    assert np.all((xs >= 0) & (xs < Nc))
+    got = dict(zip(tg.tolist(), xs.tolist()))
+    assert got == {2.0: 8.5, 3.0: 0.0, 5.0: 0.0, 6.0: 1.0}                 # x' = 0 survives (cell 0)
+    keys = o.debug_get(O.KEYS)
+    assert sorted(keys.tolist()) == [-1, -1, -1, 0, 0, 1, 8]
+
+
+def test_periodic_wrap():
+    Nc = 16
+    o = O.Oracle(_one_species(Nc, 0.0, bc=1))
+    x0 = np.array([0.5, 15.5, 8.0], np.float32)
+    v0 = np.array([-1.0, 1.0, 0.5], np.float32)
+    load(o, [(x0, v0, 0 * x0, 0 * x0)])
+    o.set_E32(np.zeros(Nc, np.float32))
+    o.step(1)
+    assert sorted(o.debug_get(O.X).tolist()) == [0.5, 8.5, 15.5]
+    assert o.moments(0)["count"] == 3
+
+
+def test_secondary_emission_binomial_and_placement():
+    Nc, n = 64, 40000
+    p = params(2, n_cells=Nc, ppc=1, mcc=False, gamma=0.1, capacity_factor=2000)
+    o = O.Oracle(p)
+    rng = np.random.default_rng(1)
+    xi = np.where(np.arange(n) % 2 == 0, 0.5, Nc - 0.5).astype(np.float32)
+    vi = np.where(np.arange(n) % 2 == 0, -1.0, 1.0).astype(np.float32)     # every ion hits a wall
+    z = np.zeros(0, np.float32)
+    load(o, [(z, z, z, z), (xi, vi, 0 * xi, 0 * xi)])
+    o.set_E32(np.zeros(Nc + 1, np.float32))
+    o.step(1)
+    me, mi = o.moments(0), o.moments(1)
+    assert mi["absorbed_left"] == n // 2 and mi["absorbed_right"] == n // 2 and mi["count"] == 0
+    k = me["injected"]
+    assert k == me["count"] and abs(k - 0.1 * n) < 4 * np.sqrt(n * 0.1 * 0.9)
+    x, vx = o.debug_get(O.X), o.debug_get(O.VX)
+    left = x < 1
+    assert np.all(left | (x >= Nc - 1)) and np.all(x < Nc) and np.all(x >= 0)
+    assert np.all(vx[left] >= 0) and np.all(vx[~left] <= 0)                # pointing into the plasma
+    assert abs(left.mean() - 0.5) < 0.06
+    vy = o.debug_get(O.VY)
+    # vx = vth sqrt(-2 ln(1-u)) is Rayleigh (flux-weighted half-Maxwellian): <vx^2> = 2 vth^2,
+    # <|vx|> = vth sqrt(pi/2); (vy, vz) is a 2-D Maxwellian: <vy^2> = vth^2
+    assert abs(np.mean(vx.astype(np.float64) ** 2) / (2 * p["see_vth"] ** 2) - 1) < 0.1
+    assert abs(np.mean(np.abs(vx)) / (p["see_vth"] * np.sqrt(np.pi / 2)) - 1) < 0.05
+    assert abs(np.mean(vy.astype(np.float64) ** 2) / p["see_vth"] ** 2 - 1) < 0.1
+    assert abs(np.mean(vy)) < 4 * p["see_vth"] / np.sqrt(k)
+
+
+# ---- P8 sort ---------------------------------------------------------------------------------
+@pytest.mark.parametrize("inv_ratio", [2.0, 1.0, 0.5, 0.0625])
+def test_sort_is_stable_permutation_with_bruteforce_offsets(inv_ratio):
+    Nc, n = 32, 3000
+    rng = np.random.default_rng(11)
+    o = O.Oracle(_one_species(Nc, 0.0, inv_ratio=inv_ratio))
+    x0 = (rng.random(n, dtype=np.float32) * Nc).astype(np.float32)
+    x0[:5] = [0.0, 31.999, 16.0, 15.999, 0.5]
+    v0 = rng.normal(size=n).astype(np.float32) * 3
+    tag = np.arange(n, dtype=np.float32)
+    load(o, [(x0, v0, tag, -tag)])
+    o.set_E32(np.zeros(Nc + 1, np.float32))
+    # after load: stable sort of the input by key
+    for it in range(2):
+        xs, vs, tg, tz = (o.debug_get(w) for w in (O.X, O.VX, O.VY, O.VZ))
+        off = o.debug_get(O.OFFSETS)
+        n_sc = int(np.ceil(Nc * inv_ratio))
+        assert off.shape[0] == n_sc + 1 and off[0] == 0 and off[-1] == xs.shape[0]
+        keys = np.floor(xs.astype(np.float64) * inv_ratio).astype(np.int64)
+        assert np.all(np.diff(keys) >= 0)
+        assert np.array_equal(off, [(keys < k).sum() for k in range(n_sc + 1)])
+        assert np.array_equal(tg, -tz)                         # 4-tuples stay together
+        if it == 0:
+            assert np.array_equal(np.sort(tg), tag)            # permutation
+            for k in range(n_sc):
+                seg = tg[off[k]:off[k + 1]]
+                assert np.all(np.diff(seg) > 0)                # stable: source order kept
+            order = np.argsort(np.floor(x0.astype(np.float64) * inv_ratio), kind="stable")
+            assert np.array_equal(tg, tag[order]) and np.array_equal(xs, x0[order])
+            prev = (xs.copy(), vs.copy(), tg.copy())
+            o.step(1)
+        else:
+            # second pass: survivors of a real push, again stable w.r.t. the previous order
+            px, pv, pt = prev
+            nx = px + pv
+            alive = (nx >= 0) & (nx < Nc)
+            order = np.argsort(np.floor(nx[alive].astype(np.float64) * inv_ratio), kind="stable")
+            assert np.array_equal(tg, pt[alive][order]) and np.array_equal(xs, nx[alive][order])
