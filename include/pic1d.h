@@ -1,0 +1,175 @@
+/*
+ * pic1d.h -- C-ABI of the B200-native 1D3V electrostatic PIC/MCC hot path with per-cell fine
+ * sorting (Mertmann et al., arXiv:1104.3998; citations are PAPER.md lines).
+ *
+ * One handle = one simulation on one GPU.  All device memory is a single caller-owned workspace
+ * (e.g. a torch.empty(uint8) tensor); the library never allocates device memory.  All kernels are
+ * enqueued on the caller's stream.  A handle is used by one host thread at a time.  Every function
+ * returns 0 on success or a negative PIC1D_ERR_* code; no C++ types or exceptions cross the boundary.
+ *
+ * Units are the paper's normalised units (section 3.3): x in grid cells, t in steps,
+ * v in cells/step, rho in super-particle charges per cell, phi in Q dx/(eps0 A_e), E in Q/(eps0 A_e).
+ *
+ * One call of pic1d_step(h, 1) is one pass of the cycle of Fig. 1 (L35-41), entered at the pusher:
+ *   gather + leapfrog push (L35, L150-156, Eq. 3-4)  ->  wall absorption / secondary emission /
+ *   compaction (L41)  ->  fine sort by sort cell (L63-67, L160-192)  ->  charge deposition over the
+ *   sorted ranges (L128-138)  ->  Poisson + E (Eq. 1-2)  ->  null-collision MCC (L196-209).
+ */
+#ifndef PIC1D_H_
+#define PIC1D_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PIC1D_MAX_SPECIES 2
+
+#define PIC1D_OK 0
+#define PIC1D_ERR_ARG (-1)       /* bad argument / bad struct_size / call order */
+#define PIC1D_ERR_CAPACITY (-2)  /* sticky: a load, a birth or an injection exceeded a capacity;   \
+                                    the extra particles were dropped and counted */
+#define PIC1D_ERR_CUDA (-3)      /* a CUDA call failed; see pic1d_last_cuda_error */
+#define PIC1D_ERR_NONFINITE (-4) /* sticky: a NaN position was seen (treated as absorbed) */
+#define PIC1D_ERR_WORKSPACE (-5) /* workspace too small / sort bookkeeping pool exhausted (sticky) */
+
+/* flags */
+#define PIC1D_FLAG_CAPTURE 1u /* keep per-slot pre-sort keys and MCC event masks for pic1d_debug_get */
+
+typedef struct pic1d pic1d_t; /* opaque */
+
+typedef struct pic1d_species_config {
+    double kappa;       /* signed push constant kappa_s = sign(q) Q^2 dt^2/(eps0 dx M A_e), Eq. 3 (L119) */
+    double c_eV;        /* eV per (cell/step)^2: E = c_eV |v|^2 */
+    double P0;          /* null-collision probability P0 = 1 - exp(-dt nu_0), Eq. 6 (L200) */
+    double inv_g_cap;   /* 1/g_cap [steps/cell]; g_cap = speed at which nu(g) reaches nu_0 */
+    int64_t capacity;   /* slots per particle array; state + sort buffer are sized from it */
+    int32_t charge_sign; /* +1 / -1 */
+    int32_t mcc_kind;   /* 0 none, 1 electron set (elastic, excitation, ionisation), 2 ion charge exchange */
+} pic1d_species_config_t;
+
+typedef struct pic1d_config {
+    uint32_t struct_size; /* = sizeof(pic1d_config_t) */
+    int32_t n_cells;      /* N_c grid cells; bounded: N_c + 1 nodes, periodic: N_c nodes */
+    int32_t bc;           /* 0 bounded with absorbing walls, 1 periodic */
+    int32_t n_species;    /* 1 or 2; species 0 = electrons, species 1 = ions */
+    pic1d_species_config_t sp[PIC1D_MAX_SPECIES];
+    double background_rho; /* fixed neutralising background added to rho (periodic runs) */
+    double sort_inv_ratio; /* 1/r, r = sort-cell size / grid-cell size, a power of two (L65, L215) */
+    double V0_norm;        /* wall potential phi_0(t) = V0_norm sin(omega_dt * n); phi_{N_c} = 0 */
+    double omega_dt;
+    double see_gamma;      /* secondary-electron yield per absorbed ion (L41) */
+    double see_vth;        /* thermal speed of emitted electrons [cells/step] */
+    double r_el, r_exc, r_ion; /* sigma_el, sigma_exc0, sigma_ion0 over sigma_cap */
+    double E_exc, E_ion;   /* thresholds [eV] */
+    double gas_vth_ion;    /* thermal speed of the background gas for ion products [cells/step] */
+    double mass_ratio;     /* m_e / M */
+    uint64_t seed;         /* Philox key */
+    uint32_t flags;        /* PIC1D_FLAG_* */
+    uint32_t pad_;
+} pic1d_config_t;
+
+typedef struct pic1d_moments {
+    int64_t count;    /* live particles N_s (sorted part + this step's birth tail) */
+    int64_t n_sorted; /* sorted part */
+    double sum_vx, sum_vy, sum_vz, sum_v2, sum_v4; /* fp64 sums over all live particles */
+    int64_t absorbed_left, absorbed_right;        /* cumulative since load */
+    int64_t injected;     /* cumulative secondary electrons injected into this species */
+    int64_t n_candidates; /* cumulative particles that passed the null test (Eq. 6) */
+    int64_t n_events[4];  /* cumulative [0] null, [1] elastic or CX, [2] excitation, [3] ionisation */
+    int64_t births;       /* cumulative ionisation births appended to this species */
+    int64_t dropped;      /* cumulative births / injections dropped for lack of capacity */
+    int64_t over_cap;     /* cumulative candidates with g > g_cap */
+} pic1d_moments_t;
+
+/*
+ * Size query: bytes of device workspace pic1d_create needs for this config.  HOST pointers.
+ */
+int pic1d_workspace_bytes(const pic1d_config_t* cfg, size_t* bytes_out);
+
+/*
+ * Create a handle.  cfg: HOST pointer, copied.  workspace: DEVICE memory, 256-byte aligned, at least
+ * pic1d_workspace_bytes() long, owned by the caller and kept alive until pic1d_destroy.
+ * cuda_stream: the caller's cudaStream_t (NULL = default stream).  *out receives the handle.
+ * (Problem statement L33-41; data structure L63-67.)
+ */
+int pic1d_create(const pic1d_config_t* cfg, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                 pic1d_t** out);
+
+/*
+ * Load species `species` (L63): n particles, x in [0, N_c) grid-cell units, velocities in cells/step
+ * taken as v(-dt/2) (leapfrog, L150).  Arrays are HOST (on_device = 0) or DEVICE (on_device = 1)
+ * fp32, copied; the caller keeps ownership.  When the last species has been loaded the library
+ * fine-sorts, deposits and solves, so rho/phi/E are valid for step 0 and the step counter is 0.
+ * n > capacity -> PIC1D_ERR_CAPACITY; x outside [0, N_c) -> PIC1D_ERR_ARG (checked on the device).
+ */
+int pic1d_load_particles(pic1d_t* h, int species, int64_t n, const float* x, const float* vx,
+                         const float* vy, const float* vz, int on_device);
+
+/*
+ * Enqueue n_steps full PIC/MCC cycles (Fig. 1, L35-41) on the stream.  Asynchronous: no host
+ * synchronisation, no host round trip of rho or E (contrast L144).  Errors raised inside the
+ * kernels are sticky and surface on the next synchronising call.
+ */
+int pic1d_step(pic1d_t* h, int n_steps);
+
+/*
+ * Copy net charge density rho (raw linear-weighting sums, no wall-node doubling), potential phi and
+ * field E (Eq. 1-2), fp64, n_nodes values each, to HOST (on_device = 0; synchronises) or
+ * DEVICE (on_device = 1; enqueued) buffers.  Any pointer may be NULL.  Returns the sticky error.
+ */
+int pic1d_get_rho_phi_E(pic1d_t* h, double* rho, double* phi, double* E, int n_nodes, int on_device);
+
+/*
+ * Moments of species `species` (synchronises).  out: HOST.  density: optional HOST buffer of
+ * n_density = n_nodes doubles receiving rho_s of the last deposit (number density per node).
+ * eedf: optional HOST buffer of n_bins int64 receiving the histogram of E = c_eV |v|^2 on [0, E_max).
+ */
+int pic1d_moments(pic1d_t* h, int species, pic1d_moments_t* out, double* density, int n_density,
+                  int64_t* eedf, int n_bins, double E_max);
+
+/* Free the host-side handle.  The workspace stays the caller's. */
+int pic1d_destroy(pic1d_t* h);
+
+/* ---- helpers outside the six-call contract ------------------------------------------------- */
+int pic1d_n_nodes(const pic1d_t* h);
+int pic1d_n_sort_cells(const pic1d_t* h);
+uint32_t pic1d_step_index(const pic1d_t* h);
+const char* pic1d_last_cuda_error(const pic1d_t* h);
+/* number of kernel launches enqueued by this handle since creation */
+int64_t pic1d_launch_count(const pic1d_t* h);
+
+/* Per-kernel timing (host API, synchronises): runs ONE step with CUDA events between the kernels
+ * and writes up to max_kernels entries of (name, milliseconds).  Returns the number of entries. */
+typedef struct pic1d_kernel_time {
+    char name[48];
+    float ms;
+    int32_t species; /* -1 = not species specific */
+} pic1d_kernel_time_t;
+int pic1d_step_timed(pic1d_t* h, pic1d_kernel_time_t* out, int max_kernels);
+
+/* Debug access for the parity harness (synchronises).  `what` selects the array; *count_out gets
+ * the element count; dst (HOST) must hold `bytes` >= count * element size. */
+enum pic1d_debug_what {
+    PIC1D_DBG_X = 0,   /* float[N_s]  */
+    PIC1D_DBG_VX = 1,
+    PIC1D_DBG_VY = 2,
+    PIC1D_DBG_VZ = 3,
+    PIC1D_DBG_KEYS = 4,    /* int32 per pre-sort slot of the last step, -1 = absorbed (needs CAPTURE) */
+    PIC1D_DBG_OFFSETS = 5, /* int32[N_sc + 1] */
+    PIC1D_DBG_MASK = 6,    /* uint8 per sorted slot: MCC event of the last step (needs CAPTURE) */
+    PIC1D_DBG_E32 = 7,     /* float[n_nodes]: the field the next push will gather */
+    PIC1D_DBG_RHO_S = 8    /* double[n_nodes]: rho_s of the last deposit */
+};
+int pic1d_debug_count(pic1d_t* h, int what, int species, int64_t* count_out);
+int pic1d_debug_get(pic1d_t* h, int what, int species, void* dst, size_t bytes);
+/* Overwrite the fp32 field the next push gathers (so a single-step parity test can start from an
+ * identical state, R17).  E32: HOST, n_nodes floats. */
+int pic1d_debug_set_E32(pic1d_t* h, const float* E32, int n_nodes);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIC1D_H_ */

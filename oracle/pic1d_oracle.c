@@ -463,7 +463,8 @@ static void step_once(orc_t* o) {
             if (c->bc == 1) {
                 if (x < 0.0f) x += fNc;
                 if (x >= fNc) x -= fNc;
-                if (x >= fNc) x = 0.0f;
+                /* rounding of -tiny + N_c, |v| > N_c, or non-finite: back to x = 0 */
+                if (!(x >= 0.0f && x < fNc)) x = 0.0f;
             } else if (!(x >= 0.0f && x < fNc)) {
                 if (x != x) o->error = -4;
                 if (x < 0.0f) p->m.absorbed_left++; else p->m.absorbed_right++;

@@ -1,0 +1,591 @@
+// pic1d.cu -- C-ABI (include/pic1d.h) and step orchestration of the B200-native PIC/MCC hot path.
+//
+// One stream-ordered kernel sequence per step, no host round trip (contrast PAPER.md L144):
+//   k_step_begin
+//   per species (ions first, so their wall hits can emit secondaries into the electron source):
+//       k_push_count -> k_bin_scan -> k_offsets_scan -> k_push_scatter [-> k_see_emit]
+//   k_deposit per species -> k_rho_combine -> k_field -> k_mcc per species
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -fmad=false (see ../build.py).
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/pic1d.h"
+#include "pic1d_device.cuh"
+#include "pic1d_sort.cuh"
+#include "pic1d_grid.cuh"
+#include "pic1d_mcc.cuh"
+
+namespace {
+
+struct SpeciesHost {
+    float* buf[2][4];
+    int cur;
+    int capacity, n_tiles_max, n_groups_max;
+    int *tile_lo, *tile_w, *tile_off, *tile_dead, *grp_lo, *grp_hi, *pool;
+    int pool_size;
+    int *hist, *offsets, *keys_dbg;
+    uint8_t* mask;
+    double *part, *side, *rho_s;
+    ull* desc;
+    int n_mcc_tiles;
+};
+
+struct TimeMark {
+    const char* name;
+    int species;
+    cudaEvent_t ev;
+};
+
+}  // namespace
+
+struct pic1d {
+    pic1d_config_t cfg;
+    cudaStream_t stream;
+    int nodes, n_sc, T, G, n_dep_blocks, num_sms;
+    float inv_r;
+    SpeciesHost sp[2];
+    DevState* st;
+    double *rho, *phi, *E, *S, *Tt, *mom_partial;
+    float* E32;
+    unsigned* abs_list;
+    int abs_cap;
+    ull* eedf_dev;
+    int eedf_cap;
+    uint32_t step;
+    int loaded_mask;
+    bool ready;
+    int64_t launches;
+    cudaError_t last_err;
+    int grid_count, grid_scatter;
+    size_t smem_sort;
+    bool timing;
+    std::vector<TimeMark> marks;
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used;
+};
+
+namespace {
+
+const int MOM_BLOCKS = 1024;
+const int EEDF_MAX_BINS = 65536;
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+template <class Tp>
+Tp* carve(char* base, size_t& off, size_t count) {
+    off = align_up(off, 256);
+    Tp* p = base ? reinterpret_cast<Tp*>(base + off) : nullptr;
+    off += count * sizeof(Tp);
+    return p;
+}
+
+int pow2_floor(int v) {
+    int p = 1;
+    while (p * 2 <= v) p *= 2;
+    return p;
+}
+
+int validate_cfg(const pic1d_config_t* c) {
+    if (!c || c->struct_size != sizeof(pic1d_config_t)) return PIC1D_ERR_ARG;
+    if (c->n_cells < 2 || c->n_cells > (1 << 24)) return PIC1D_ERR_ARG;
+    if (c->bc != 0 && c->bc != 1) return PIC1D_ERR_ARG;
+    if (c->n_species < 1 || c->n_species > PIC1D_MAX_SPECIES) return PIC1D_ERR_ARG;
+    if (!(c->sort_inv_ratio > 0.0)) return PIC1D_ERR_ARG;
+    int e;
+    double m = std::frexp(c->sort_inv_ratio, &e);
+    if (m != 0.5) return PIC1D_ERR_ARG;  // power of two: x * inv_r is exact (R9)
+    double nsc = std::ceil((double)c->n_cells * c->sort_inv_ratio);
+    if (nsc < 1 || nsc > 49152) return PIC1D_ERR_ARG;  // one int counter per sort cell in shared memory
+    for (int s = 0; s < c->n_species; ++s) {
+        int64_t cap = c->sp[s].capacity;
+        if (cap < 4096 || cap % 4096 != 0 || cap > (1ll << 30)) return PIC1D_ERR_ARG;
+    }
+    return PIC1D_OK;
+}
+
+// Lay the handle's device arrays out in the caller's workspace (base == nullptr: size query only).
+size_t layout(pic1d* h, char* base) {
+    const pic1d_config_t& c = h->cfg;
+    h->nodes = c.bc == 1 ? c.n_cells : c.n_cells + 1;
+    h->n_sc = (int)std::ceil((double)c.n_cells * c.sort_inv_ratio);
+    h->inv_r = (float)c.sort_inv_ratio;
+    int64_t cap_max = 0;
+    for (int s = 0; s < c.n_species; ++s) cap_max = std::max<int64_t>(cap_max, c.sp[s].capacity);
+    h->T = cap_max >= 4096ll * 592 ? 4096 : (cap_max >= 2048ll * 592 ? 2048 : 1024);
+    const int rr = c.sort_inv_ratio < 1.0 ? (int)std::llround(1.0 / c.sort_inv_ratio) : 1;
+    const int ppc_est = (int)std::max<int64_t>(1, cap_max / c.n_cells);
+    h->G = std::min(2048, std::max(rr, pow2_floor(std::max(1, 4096 / ppc_est))));
+    h->n_dep_blocks = (c.n_cells + h->G - 1) / h->G;
+    size_t off = 0;
+    h->st = carve<DevState>(base, off, 1);
+    h->rho = carve<double>(base, off, h->nodes + 1);
+    h->phi = carve<double>(base, off, h->nodes + 1);
+    h->E = carve<double>(base, off, h->nodes + 1);
+    h->S = carve<double>(base, off, h->nodes + 1);
+    h->Tt = carve<double>(base, off, h->nodes + 1);
+    h->E32 = carve<float>(base, off, h->nodes + 1);
+    h->mom_partial = carve<double>(base, off, MOM_BLOCKS * 5);
+    h->eedf_cap = EEDF_MAX_BINS;
+    h->eedf_dev = carve<ull>(base, off, EEDF_MAX_BINS);
+    h->abs_cap = 0;
+    h->abs_list = nullptr;
+    if (c.n_species > 1 && c.see_gamma > 0.0 && c.bc == 0) {
+        h->abs_cap = (int)std::min<int64_t>(c.sp[1].capacity, std::max<int64_t>(1 << 20, c.sp[1].capacity / 16));
+        h->abs_list = carve<unsigned>(base, off, h->abs_cap);
+    }
+    for (int s = 0; s < c.n_species; ++s) {
+        SpeciesHost& p = h->sp[s];
+        p.capacity = (int)c.sp[s].capacity;
+        p.cur = 0;
+        for (int b = 0; b < 2; ++b)
+            for (int k = 0; k < 4; ++k) p.buf[b][k] = carve<float>(base, off, p.capacity);
+        p.n_tiles_max = p.capacity / h->T;
+        p.n_groups_max = (p.n_tiles_max + PIC1D_GROUP - 1) / PIC1D_GROUP;
+        p.tile_lo = carve<int>(base, off, p.n_tiles_max);
+        p.tile_w = carve<int>(base, off, p.n_tiles_max);
+        p.tile_off = carve<int>(base, off, p.n_tiles_max);
+        p.tile_dead = carve<int>(base, off, p.n_tiles_max);
+        p.grp_lo = carve<int>(base, off, p.n_groups_max);
+        p.grp_hi = carve<int>(base, off, p.n_groups_max);
+        int64_t full = (int64_t)p.n_tiles_max * h->n_sc;
+        int64_t want = std::max<int64_t>(1 << 20, (int64_t)p.n_tiles_max * 4096);
+        p.pool_size = (int)std::min<int64_t>(std::min(full, want), (1ll << 30));
+        p.pool = carve<int>(base, off, p.pool_size);
+        p.hist = carve<int>(base, off, h->n_sc + 1);
+        p.offsets = carve<int>(base, off, h->n_sc + 1);
+        p.keys_dbg = nullptr;
+        p.mask = nullptr;
+        if (c.flags & PIC1D_FLAG_CAPTURE) {
+            p.keys_dbg = carve<int>(base, off, p.capacity);
+            p.mask = carve<uint8_t>(base, off, p.capacity);
+        }
+        p.part = carve<double>(base, off, (size_t)h->n_dep_blocks * h->G);
+        p.side = carve<double>(base, off, h->n_dep_blocks);
+        p.rho_s = carve<double>(base, off, h->nodes + 1);
+        p.n_mcc_tiles = (p.capacity + MCC_TILE - 1) / MCC_TILE;
+        p.desc = carve<ull>(base, off, p.n_mcc_tiles);
+    }
+    return align_up(off, 256);
+}
+
+bool ck(pic1d* h, cudaError_t e) {
+    if (e != cudaSuccess) { h->last_err = e; return false; }
+    return true;
+}
+
+void mark(pic1d* h, const char* name, int species) {
+    h->launches++;
+    if (!h->timing) return;
+    if (h->ev_used == h->ev_pool.size()) {
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        h->ev_pool.push_back(e);
+    }
+    cudaEvent_t e = h->ev_pool[h->ev_used++];
+    cudaEventRecord(e, h->stream);
+    h->marks.push_back(TimeMark{name, species, e});
+}
+
+SortArgs sort_args(pic1d* h, int s) {
+    SpeciesHost& p = h->sp[s];
+    SortArgs a;
+    const int c = p.cur, d = c ^ 1;
+    a.sx = p.buf[c][0]; a.svx = p.buf[c][1]; a.svy = p.buf[c][2]; a.svz = p.buf[c][3];
+    a.dx = p.buf[d][0]; a.dvx = p.buf[d][1]; a.dvy = p.buf[d][2]; a.dvz = p.buf[d][3];
+    a.E32 = h->E32; a.st = h->st; a.s = s;
+    a.tile_lo = p.tile_lo; a.tile_w = p.tile_w; a.tile_off = p.tile_off; a.tile_dead = p.tile_dead;
+    a.grp_lo = p.grp_lo; a.grp_hi = p.grp_hi; a.pool = p.pool; a.pool_size = p.pool_size;
+    a.hist = p.hist; a.offsets = p.offsets; a.keys_dbg = p.keys_dbg;
+    a.abs_list = (s == 1) ? h->abs_list : nullptr;
+    a.abs_cap = h->abs_cap;
+    a.kappa = (float)h->cfg.sp[s].kappa;
+    a.fNc = (float)h->cfg.n_cells; a.inv_r = h->inv_r; a.Nc = h->cfg.n_cells; a.n_sc = h->n_sc;
+    return a;
+}
+
+template <int BC>
+void launch_count(pic1d* h, const SortArgs& a, int grid) {
+    switch (h->T) {
+        case 4096: k_push_count<BC, 4><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
+        case 2048: k_push_count<BC, 2><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
+        default: k_push_count<BC, 1><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
+    }
+}
+template <int BC>
+void launch_scatter(pic1d* h, const SortArgs& a, int grid) {
+    switch (h->T) {
+        case 4096: k_push_scatter<BC, 16><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
+        case 2048: k_push_scatter<BC, 8><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
+        default: k_push_scatter<BC, 4><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
+    }
+}
+
+template <class K>
+int occupancy_grid(pic1d* h, K kernel, size_t smem) {
+    if (smem > 48 * 1024) cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    int nb = 1;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, PIC1D_NT, smem);
+    return std::max(1, nb) * h->num_sms;
+}
+
+void setup_launch(pic1d* h) {
+    const size_t smem = (size_t)h->n_sc * sizeof(int);
+    h->smem_sort = smem;
+    int gc, gs;
+    if (h->cfg.bc == 1) {
+        if (h->T == 4096) { gc = occupancy_grid(h, k_push_count<1, 4>, smem); gs = occupancy_grid(h, k_push_scatter<1, 16>, smem); }
+        else if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<1, 2>, smem); gs = occupancy_grid(h, k_push_scatter<1, 8>, smem); }
+        else { gc = occupancy_grid(h, k_push_count<1, 1>, smem); gs = occupancy_grid(h, k_push_scatter<1, 4>, smem); }
+    } else {
+        if (h->T == 4096) { gc = occupancy_grid(h, k_push_count<0, 4>, smem); gs = occupancy_grid(h, k_push_scatter<0, 16>, smem); }
+        else if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<0, 2>, smem); gs = occupancy_grid(h, k_push_scatter<0, 8>, smem); }
+        else { gc = occupancy_grid(h, k_push_count<0, 1>, smem); gs = occupancy_grid(h, k_push_scatter<0, 4>, smem); }
+    }
+    h->grid_count = gc;
+    h->grid_scatter = gs;
+}
+
+// fine sort of species s (mode 0: no push)
+void enqueue_sort(pic1d* h, int s) {
+    SpeciesHost& p = h->sp[s];
+    SortArgs a = sort_args(h, s);
+    const int gc = std::min(h->grid_count, p.n_tiles_max), gs = std::min(h->grid_scatter, p.n_tiles_max);
+    if (h->cfg.bc == 1) launch_count<1>(h, a, gc); else launch_count<0>(h, a, gc);
+    mark(h, "push_count", s);
+    k_bin_scan<<<(h->n_sc + 127) / 128, 128, 0, h->stream>>>(a);
+    mark(h, "bin_scan", s);
+    k_offsets_scan<<<1, 1024, 0, h->stream>>>(a);
+    mark(h, "offsets_scan", s);
+    if (h->cfg.bc == 1) launch_scatter<1>(h, a, gs); else launch_scatter<0>(h, a, gs);
+    mark(h, "push_scatter", s);
+    p.cur ^= 1;
+}
+
+void enqueue_begin(pic1d* h, int mode) {
+    const int ns = h->cfg.n_species;
+    k_step_begin<<<4, 256, 0, h->stream>>>(h->st, ns, mode, h->T, h->sp[0].grp_lo, h->sp[0].grp_hi,
+                                           ns > 1 ? h->sp[1].grp_lo : nullptr, ns > 1 ? h->sp[1].grp_hi : nullptr,
+                                           h->sp[0].n_groups_max, ns > 1 ? h->sp[1].n_groups_max : 0);
+    mark(h, "step_begin", -1);
+}
+
+void enqueue_grid(pic1d* h, unsigned n_time) {
+    const pic1d_config_t& c = h->cfg;
+    CombineArgs cb;
+    memset(&cb, 0, sizeof(cb));
+    for (int s = 0; s < c.n_species; ++s) {
+        SpeciesHost& p = h->sp[s];
+        DepositArgs d;
+        d.x = p.buf[p.cur][0]; d.offsets = p.offsets; d.part = p.part; d.side = p.side;
+        d.Nc = c.n_cells; d.n_sc = h->n_sc; d.G = h->G; d.inv_r = h->inv_r;
+        k_deposit<<<h->n_dep_blocks, PIC1D_NT, (h->G + 1) * sizeof(double), h->stream>>>(d);
+        mark(h, "deposit", s);
+        cb.part[s] = p.part; cb.side[s] = p.side; cb.rho_s[s] = p.rho_s; cb.sign[s] = c.sp[s].charge_sign;
+    }
+    cb.rho = h->rho; cb.n_species = c.n_species; cb.Nc = c.n_cells; cb.nodes = h->nodes; cb.G = h->G;
+    cb.bc = c.bc; cb.background = c.background_rho;
+    k_rho_combine<<<(h->nodes + 255) / 256, 256, 0, h->stream>>>(cb);
+    mark(h, "rho_combine", -1);
+    FieldArgs f;
+    f.rho = h->rho; f.phi = h->phi; f.E = h->E; f.S = h->S; f.Tt = h->Tt; f.E32 = h->E32;
+    f.Nc = c.n_cells; f.nodes = h->nodes; f.bc = c.bc; f.V0 = c.V0_norm; f.omega_dt = c.omega_dt;
+    f.n_time = n_time;
+    k_field<<<1, 1024, 0, h->stream>>>(f);
+    mark(h, "field", -1);
+}
+
+void enqueue_mcc(pic1d* h) {
+    const pic1d_config_t& c = h->cfg;
+    for (int s = 0; s < c.n_species; ++s) {
+        if (c.sp[s].mcc_kind == 0) continue;
+        SpeciesHost& p = h->sp[s];
+        SpeciesHost& pe = h->sp[0];
+        MccArgs m;
+        memset(&m, 0, sizeof(m));
+        m.x = p.buf[p.cur][0]; m.vx = p.buf[p.cur][1]; m.vy = p.buf[p.cur][2]; m.vz = p.buf[p.cur][3];
+        m.ex = pe.buf[pe.cur][0]; m.evx = pe.buf[pe.cur][1]; m.evy = pe.buf[pe.cur][2]; m.evz = pe.buf[pe.cur][3];
+        m.cap_e = pe.capacity;
+        if (c.n_species > 1) {
+            SpeciesHost& pi = h->sp[1];
+            m.ix = pi.buf[pi.cur][0]; m.ivx = pi.buf[pi.cur][1]; m.ivy = pi.buf[pi.cur][2]; m.ivz = pi.buf[pi.cur][3];
+            m.cap_i = pi.capacity;
+        }
+        m.st = h->st; m.desc = p.desc; m.mask = p.mask;
+        m.s = s; m.kind = c.sp[s].mcc_kind; m.n_species = c.n_species;
+        m.step = h->step; m.k0 = (uint32_t)c.seed; m.k1 = (uint32_t)(c.seed >> 32);
+        m.P0 = (float)c.sp[s].P0; m.inv_g_cap = (float)c.sp[s].inv_g_cap; m.c_eV = (float)c.sp[s].c_eV;
+        m.r_el = (float)c.r_el; m.r_exc = (float)c.r_exc; m.r_ion = (float)c.r_ion;
+        m.E_exc = (float)c.E_exc; m.E_ion = (float)c.E_ion;
+        m.two_mr = (float)(2.0 * c.mass_ratio); m.gvt = (float)c.gas_vth_ion;
+        k_mcc<<<p.n_mcc_tiles, PIC1D_NT, 0, h->stream>>>(m);
+        mark(h, "mcc", s);
+    }
+}
+
+void enqueue_step(pic1d* h) {
+    const pic1d_config_t& c = h->cfg;
+    enqueue_begin(h, 1);
+    if (c.n_species > 1) {
+        enqueue_sort(h, 1);
+        if (h->abs_list) {
+            SpeciesHost& pe = h->sp[0];
+            SeeArgs sa;
+            sa.st = h->st; sa.abs_list = h->abs_list; sa.abs_cap = h->abs_cap;
+            sa.ex = pe.buf[pe.cur][0]; sa.evx = pe.buf[pe.cur][1]; sa.evy = pe.buf[pe.cur][2]; sa.evz = pe.buf[pe.cur][3];
+            sa.cap_e = pe.capacity; sa.T = h->T;
+            sa.gamma = (float)c.see_gamma; sa.vth = (float)c.see_vth; sa.fNc = (float)c.n_cells;
+            sa.k0 = (uint32_t)c.seed; sa.k1 = (uint32_t)(c.seed >> 32); sa.step = h->step;
+            k_see_emit<<<1, 1024, 0, h->stream>>>(sa);
+            mark(h, "see_emit", 0);
+        }
+    }
+    enqueue_sort(h, 0);
+    enqueue_grid(h, h->step + 1u);
+    enqueue_mcc(h);
+    h->step += 1u;
+}
+
+int sticky_code(unsigned err) {
+    if (err & ERRBIT_NONFINITE) return PIC1D_ERR_NONFINITE;
+    if (err & ERRBIT_CAPACITY) return PIC1D_ERR_CAPACITY;
+    if (err & ERRBIT_WORKSPACE) return PIC1D_ERR_WORKSPACE;
+    if (err & ERRBIT_BADLOAD) return PIC1D_ERR_ARG;
+    return PIC1D_OK;
+}
+
+int fetch_state(pic1d* h, DevState* out) {
+    if (!ck(h, cudaMemcpyAsync(out, h->st, sizeof(DevState), cudaMemcpyDeviceToHost, h->stream))) return PIC1D_ERR_CUDA;
+    if (!ck(h, cudaStreamSynchronize(h->stream))) return PIC1D_ERR_CUDA;
+    return PIC1D_OK;
+}
+
+__global__ void k_set_count(DevState* st, int s, int n) {
+    DevSpecies& sp = st->sp[s];
+    memset(&sp, 0, sizeof(sp));
+    sp.n_live = n;
+}
+__global__ void k_clear_err(DevState* st) { st->err = 0; st->step = 0; st->n_abs = 0; }
+
+}  // namespace
+
+// =================================== C-ABI ===========================================================
+extern "C" {
+
+int pic1d_workspace_bytes(const pic1d_config_t* cfg, size_t* bytes_out) {
+    if (!bytes_out) return PIC1D_ERR_ARG;
+    int rc = validate_cfg(cfg);
+    if (rc) return rc;
+    pic1d tmp{};
+    tmp.cfg = *cfg;
+    *bytes_out = layout(&tmp, nullptr);
+    return PIC1D_OK;
+}
+
+int pic1d_create(const pic1d_config_t* cfg, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                 pic1d_t** out) {
+    if (!out || !workspace) return PIC1D_ERR_ARG;
+    int rc = validate_cfg(cfg);
+    if (rc) return rc;
+    if (reinterpret_cast<uintptr_t>(workspace) % 256 != 0) return PIC1D_ERR_ARG;
+    pic1d* h = new (std::nothrow) pic1d{};
+    if (!h) return PIC1D_ERR_ARG;
+    h->cfg = *cfg;
+    h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const size_t need = layout(h, reinterpret_cast<char*>(workspace));
+    if (need > workspace_bytes) { delete h; return PIC1D_ERR_WORKSPACE; }
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        delete h;
+        return PIC1D_ERR_CUDA;
+    }
+    h->num_sms = prop.multiProcessorCount;
+    setup_launch(h);
+    h->last_err = cudaSuccess;
+    // zero the bookkeeping (state, look-back descriptors); particle arrays need no initialisation
+    bool ok = ck(h, cudaMemsetAsync(h->st, 0, sizeof(DevState), h->stream));
+    for (int s = 0; s < cfg->n_species && ok; ++s)
+        ok = ck(h, cudaMemsetAsync(h->sp[s].desc, 0, sizeof(ull) * h->sp[s].n_mcc_tiles, h->stream));
+    ok = ok && ck(h, cudaMemsetAsync(h->E32, 0, sizeof(float) * (h->nodes + 1), h->stream));
+    if (!ok || !ck(h, cudaGetLastError())) { delete h; return PIC1D_ERR_CUDA; }
+    *out = h;
+    return PIC1D_OK;
+}
+
+int pic1d_destroy(pic1d_t* h) {
+    if (!h) return PIC1D_OK;
+    cudaStreamSynchronize(h->stream);
+    for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
+    delete h;
+    return PIC1D_OK;
+}
+
+int pic1d_load_particles(pic1d_t* h, int s, int64_t n, const float* x, const float* vx, const float* vy,
+                         const float* vz, int on_device) {
+    if (!h || s < 0 || s >= h->cfg.n_species || n < 0) return PIC1D_ERR_ARG;
+    if (n > 0 && (!x || !vx || !vy || !vz)) return PIC1D_ERR_ARG;
+    SpeciesHost& p = h->sp[s];
+    if (n > p.capacity) return PIC1D_ERR_CAPACITY;
+    if (h->loaded_mask == 0) {  // a new run starts: all species must be (re)loaded
+        h->ready = false;
+        for (int q = 0; q < h->cfg.n_species; ++q) h->sp[q].cur = 0;
+        k_clear_err<<<1, 1, 0, h->stream>>>(h->st);
+        h->launches++;
+    }
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    const float* src[4] = {x, vx, vy, vz};
+    for (int k = 0; k < 4 && n > 0; ++k)
+        if (!ck(h, cudaMemcpyAsync(p.buf[0][k], src[k], (size_t)n * sizeof(float), kind, h->stream)))
+            return PIC1D_ERR_CUDA;
+    k_set_count<<<1, 1, 0, h->stream>>>(h->st, s, (int)n);
+    k_validate<<<(int)std::min<int64_t>(1024, n / 256 + 1), 256, 0, h->stream>>>(p.buf[0][0], (int)n, (float)h->cfg.n_cells, h->st);
+    h->launches += 2;
+    h->loaded_mask |= 1 << s;
+    if (h->loaded_mask != (1 << h->cfg.n_species) - 1) return ck(h, cudaGetLastError()) ? PIC1D_OK : PIC1D_ERR_CUDA;
+    // last species in: fine-sort, deposit and solve so that rho / phi / E are valid for step 0
+    h->loaded_mask = 0;
+    h->step = 0;
+    for (int q = 0; q < h->cfg.n_species; ++q) {
+        SpeciesHost& pq = h->sp[q];
+        cudaMemsetAsync(pq.desc, 0, sizeof(ull) * pq.n_mcc_tiles, h->stream);
+        if (pq.mask) cudaMemsetAsync(pq.mask, 0, pq.capacity, h->stream);
+    }
+    enqueue_begin(h, 0);
+    for (int q = h->cfg.n_species - 1; q >= 0; --q) enqueue_sort(h, q);
+    enqueue_grid(h, 0u);
+    if (!ck(h, cudaGetLastError())) return PIC1D_ERR_CUDA;
+    if (!on_device && !ck(h, cudaStreamSynchronize(h->stream))) return PIC1D_ERR_CUDA;  // host buffers may go away
+    h->ready = true;
+    return PIC1D_OK;
+}
+
+int pic1d_step(pic1d_t* h, int n_steps) {
+    if (!h || n_steps < 0 || !h->ready) return PIC1D_ERR_ARG;
+    for (int k = 0; k < n_steps; ++k) enqueue_step(h);
+    return ck(h, cudaGetLastError()) ? PIC1D_OK : PIC1D_ERR_CUDA;
+}
+
+int pic1d_step_timed(pic1d_t* h, pic1d_kernel_time_t* out, int max_kernels) {
+    if (!h || !out || max_kernels <= 0 || !h->ready) return PIC1D_ERR_ARG;
+    h->timing = true;
+    h->marks.clear();
+    h->ev_used = 0;
+    mark(h, "start", -1);
+    h->launches--;
+    enqueue_step(h);
+    h->timing = false;
+    if (!ck(h, cudaStreamSynchronize(h->stream))) return PIC1D_ERR_CUDA;
+    int n = 0;
+    for (size_t i = 1; i < h->marks.size() && n < max_kernels; ++i, ++n) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, h->marks[i - 1].ev, h->marks[i].ev);
+        snprintf(out[n].name, sizeof(out[n].name), "%s", h->marks[i].name);
+        out[n].ms = ms;
+        out[n].species = h->marks[i].species;
+    }
+    return n;
+}
+
+int pic1d_get_rho_phi_E(pic1d_t* h, double* rho, double* phi, double* E, int n_nodes, int on_device) {
+    if (!h || n_nodes != h->nodes || !h->ready) return PIC1D_ERR_ARG;
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    const size_t bytes = (size_t)n_nodes * sizeof(double);
+    if (rho && !ck(h, cudaMemcpyAsync(rho, h->rho, bytes, kind, h->stream))) return PIC1D_ERR_CUDA;
+    if (phi && !ck(h, cudaMemcpyAsync(phi, h->phi, bytes, kind, h->stream))) return PIC1D_ERR_CUDA;
+    if (E && !ck(h, cudaMemcpyAsync(E, h->E, bytes, kind, h->stream))) return PIC1D_ERR_CUDA;
+    if (on_device) return PIC1D_OK;
+    DevState st;
+    int rc = fetch_state(h, &st);
+    return rc ? rc : sticky_code(st.err);
+}
+
+int pic1d_moments(pic1d_t* h, int s, pic1d_moments_t* out, double* density, int n_density, int64_t* eedf,
+                  int n_bins, double E_max) {
+    if (!h || !out || s < 0 || s >= h->cfg.n_species || !h->ready) return PIC1D_ERR_ARG;
+    if (density && n_density != h->nodes) return PIC1D_ERR_ARG;
+    if (eedf && (n_bins <= 0 || n_bins > h->eedf_cap || !(E_max > 0.0))) return PIC1D_ERR_ARG;
+    SpeciesHost& p = h->sp[s];
+    MomArgs m;
+    m.vx = p.buf[p.cur][1]; m.vy = p.buf[p.cur][2]; m.vz = p.buf[p.cur][3];
+    m.st = h->st; m.s = s; m.partial = h->mom_partial;
+    m.eedf = eedf ? h->eedf_dev : nullptr; m.n_bins = n_bins; m.E_max = E_max; m.c_eV = h->cfg.sp[s].c_eV;
+    if (eedf) cudaMemsetAsync(h->eedf_dev, 0, sizeof(ull) * n_bins, h->stream);
+    k_moments<<<MOM_BLOCKS, 256, 0, h->stream>>>(m);
+    h->launches++;
+    std::vector<double> part(MOM_BLOCKS * 5);
+    if (!ck(h, cudaMemcpyAsync(part.data(), h->mom_partial, sizeof(double) * MOM_BLOCKS * 5, cudaMemcpyDeviceToHost, h->stream)))
+        return PIC1D_ERR_CUDA;
+    if (density && !ck(h, cudaMemcpyAsync(density, p.rho_s, sizeof(double) * h->nodes, cudaMemcpyDeviceToHost, h->stream)))
+        return PIC1D_ERR_CUDA;
+    if (eedf && !ck(h, cudaMemcpyAsync(eedf, h->eedf_dev, sizeof(ull) * n_bins, cudaMemcpyDeviceToHost, h->stream)))
+        return PIC1D_ERR_CUDA;
+    DevState st;
+    int rc = fetch_state(h, &st);
+    if (rc) return rc;
+    double acc[5] = {0, 0, 0, 0, 0};
+    for (int b = 0; b < MOM_BLOCKS; ++b)
+        for (int k = 0; k < 5; ++k) acc[k] += part[b * 5 + k];
+    const DevSpecies& d = st.sp[s];
+    memset(out, 0, sizeof(*out));
+    out->count = d.n_live; out->n_sorted = d.n_sorted;
+    out->sum_vx = acc[0]; out->sum_vy = acc[1]; out->sum_vz = acc[2]; out->sum_v2 = acc[3]; out->sum_v4 = acc[4];
+    out->absorbed_left = (int64_t)d.absorbed_left; out->absorbed_right = (int64_t)d.absorbed_right;
+    out->injected = (int64_t)d.injected; out->n_candidates = (int64_t)d.n_candidates;
+    for (int k = 0; k < 4; ++k) out->n_events[k] = (int64_t)d.n_events[k];
+    out->births = (int64_t)d.births; out->dropped = (int64_t)d.dropped; out->over_cap = (int64_t)d.over_cap;
+    return sticky_code(st.err);
+}
+
+int pic1d_n_nodes(const pic1d_t* h) { return h ? h->nodes : PIC1D_ERR_ARG; }
+int pic1d_n_sort_cells(const pic1d_t* h) { return h ? h->n_sc : PIC1D_ERR_ARG; }
+uint32_t pic1d_step_index(const pic1d_t* h) { return h ? h->step : 0u; }
+const char* pic1d_last_cuda_error(const pic1d_t* h) { return h ? cudaGetErrorString(h->last_err) : "null handle"; }
+int64_t pic1d_launch_count(const pic1d_t* h) { return h ? h->launches : 0; }
+
+int pic1d_debug_count(pic1d_t* h, int what, int s, int64_t* count_out) {
+    if (!h || !count_out || s < 0 || s >= h->cfg.n_species || !h->ready) return PIC1D_ERR_ARG;
+    DevState st;
+    int rc = fetch_state(h, &st);
+    if (rc) return rc;
+    switch (what) {
+        case PIC1D_DBG_X: case PIC1D_DBG_VX: case PIC1D_DBG_VY: case PIC1D_DBG_VZ: *count_out = st.sp[s].n_live; break;
+        case PIC1D_DBG_KEYS: *count_out = st.sp[s].n_src; break;
+        case PIC1D_DBG_OFFSETS: *count_out = h->n_sc + 1; break;
+        case PIC1D_DBG_MASK: *count_out = st.sp[s].n_sorted; break;
+        case PIC1D_DBG_E32: case PIC1D_DBG_RHO_S: *count_out = h->nodes; break;
+        default: return PIC1D_ERR_ARG;
+    }
+    return PIC1D_OK;
+}
+
+int pic1d_debug_get(pic1d_t* h, int what, int s, void* dst, size_t bytes) {
+    int64_t n = 0;
+    int rc = pic1d_debug_count(h, what, s, &n);
+    if (rc) return rc;
+    if (!dst) return PIC1D_ERR_ARG;
+    SpeciesHost& p = h->sp[s];
+    const void* src = nullptr;
+    size_t el = 4;
+    switch (what) {
+        case PIC1D_DBG_X: case PIC1D_DBG_VX: case PIC1D_DBG_VY: case PIC1D_DBG_VZ: src = p.buf[p.cur][what]; break;
+        case PIC1D_DBG_KEYS: src = p.keys_dbg; break;
+        case PIC1D_DBG_OFFSETS: src = p.offsets; break;
+        case PIC1D_DBG_MASK: src = p.mask; el = 1; break;
+        case PIC1D_DBG_E32: src = h->E32; break;
+        case PIC1D_DBG_RHO_S: src = p.rho_s; el = 8; break;
+    }
+    if (!src || bytes < (size_t)n * el) return PIC1D_ERR_ARG;
+    if (n > 0 && !ck(h, cudaMemcpyAsync(dst, src, (size_t)n * el, cudaMemcpyDeviceToHost, h->stream))) return PIC1D_ERR_CUDA;
+    return ck(h, cudaStreamSynchronize(h->stream)) ? PIC1D_OK : PIC1D_ERR_CUDA;
+}
+
+int pic1d_debug_set_E32(pic1d_t* h, const float* E32, int n_nodes) {
+    if (!h || !E32 || n_nodes != h->nodes) return PIC1D_ERR_ARG;
+    if (!ck(h, cudaMemcpyAsync(h->E32, E32, sizeof(float) * n_nodes, cudaMemcpyHostToDevice, h->stream))) return PIC1D_ERR_CUDA;
+    return ck(h, cudaStreamSynchronize(h->stream)) ? PIC1D_OK : PIC1D_ERR_CUDA;
+}
+
+}  // extern "C"

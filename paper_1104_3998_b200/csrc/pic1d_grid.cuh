@@ -1,0 +1,265 @@
+// pic1d_grid.cuh -- charge deposition over the sorted per-cell ranges (Fig. 4-5),
+// the edge-node follow-up kernel (L138) and the single-block Poisson + E solve (Eq. 1-2,
+// L142-146).  fp64 throughout; no global floating-point atomics anywhere.
+#pragma once
+#include "pic1d_device.cuh"
+
+struct DepositArgs {
+    const float* x;      // sorted positions of the species
+    const int* offsets;  // [n_sc + 1]
+    double* part;        // [n_blocks * G]   nodes c0 .. c1-1 of each block (left-closed)
+    double* side;        // [n_blocks]       right edge node c1 of each block (paper's side array, L138)
+    int Nc, n_sc, G;     // G grid cells per block (a multiple of the sort-cell size when r > 1)
+    float inv_r;
+};
+
+__device__ __forceinline__ double warp_sum_d(double v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Block b owns grid cells [b G, (b+1) G) and therefore the contiguous slot range
+// offsets[key(b G)] .. offsets[key((b+1) G)] of the sorted array.  Every warp keeps per-lane fp64
+// partial sums in registers for the cell it is currently in (the paper's register partial sums,
+// L130), reduces them with shuffles when the cell changes, and adds the two node weights to the
+// block's shared-memory window.  Rows that straddle cells are split by cell value.
+__global__ void __launch_bounds__(PIC1D_NT) k_deposit(DepositArgs a) {
+    extern __shared__ double s_acc[];  // G + 1 nodes
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    const int c0 = blockIdx.x * a.G, c1 = min(c0 + a.G, a.Nc);
+    const int k0 = (int)__fmul_rn((float)c0, a.inv_r);
+    const int k1 = c1 >= a.Nc ? a.n_sc : (int)__fmul_rn((float)c1, a.inv_r);
+    const int p0 = a.offsets[k0], p1 = a.offsets[k1];
+    for (int i = tid; i <= a.G; i += PIC1D_NT) s_acc[i] = 0.0;
+    __syncthreads();
+    int jc = -1, accn = 0;
+    double accf = 0.0;
+    for (int rb = p0 + wp * 32; rb < p1; rb += PIC1D_NT) {
+        const int i = rb + lane;
+        const bool valid = i < p1;
+        int j = -1;
+        float f = 0.0f;
+        if (valid) {
+            const float x = __ldcs(a.x + i);
+            j = (int)x;
+            f = __fsub_rn(x, (float)j);
+        }
+        unsigned rem = __ballot_sync(0xffffffffu, valid);
+        while (rem) {
+            const int jj = __shfl_sync(0xffffffffu, j, __ffs(rem) - 1);
+            const bool in = valid && j == jj;
+            const unsigned grp = __ballot_sync(0xffffffffu, in);
+            if (grp == rem) {
+                // the rest of the row is one cell: accumulate in registers
+                if (jj != jc) {
+                    if (jc >= 0) {
+                        const double F = warp_sum_d(accf);
+                        const int n = warp_sum(accn);
+                        if (lane == 0) {
+                            atomicAdd(&s_acc[jc - c0], (double)n - F);
+                            atomicAdd(&s_acc[jc + 1 - c0], F);
+                        }
+                    }
+                    jc = jj; accf = 0.0; accn = 0;
+                }
+                if (in) { accf += (double)f; ++accn; }
+            } else {
+                const double F = warp_sum_d(in ? (double)f : 0.0);
+                if (lane == 0) {
+                    atomicAdd(&s_acc[jj - c0], (double)__popc(grp) - F);
+                    atomicAdd(&s_acc[jj + 1 - c0], F);
+                }
+            }
+            rem &= ~grp;
+        }
+    }
+    if (jc >= 0) {
+        const double F = warp_sum_d(accf);
+        const int n = warp_sum(accn);
+        if (lane == 0) {
+            atomicAdd(&s_acc[jc - c0], (double)n - F);
+            atomicAdd(&s_acc[jc + 1 - c0], F);
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < a.G; i += PIC1D_NT) a.part[(size_t)blockIdx.x * a.G + i] = s_acc[i];
+    if (tid == 0) a.side[blockIdx.x] = s_acc[c1 - c0];
+}
+
+// Follow-up kernel (L138): node j of species s = block part + the left neighbour's right-edge node;
+// net rho = background + sum_s sign_s rho_s.  One thread per node.
+struct CombineArgs {
+    const double* part[2];
+    const double* side[2];
+    double* rho_s[2];
+    double* rho;
+    int sign[2];
+    int n_species, Nc, nodes, G, bc;
+    double background;
+};
+
+__global__ void k_rho_combine(CombineArgs a) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= a.nodes) return;
+    const int nb = (a.Nc + a.G - 1) / a.G;
+    double r = a.background;
+    for (int s = 0; s < a.n_species; ++s) {
+        double v = j < a.Nc ? a.part[s][j] : 0.0;  // part is indexed by node because blocks are G-aligned
+        if (j > 0 && j % a.G == 0) v += a.side[s][j / a.G - 1];
+        if (j == a.Nc) v += a.side[s][nb - 1];               // bounded: right wall node
+        if (a.bc == 1 && j == 0) v += a.side[s][nb - 1];     // periodic: node N_c == node 0
+        a.rho_s[s][j] = v;
+        r += (double)a.sign[s] * v;
+    }
+    a.rho[j] = r;
+}
+
+// ---- Poisson + E, one block --------------------------------------------------------------------
+// The tridiagonal system  phi[j-1] - 2 phi[j] + phi[j+1] = -rho[j]  (Eq. 1 discretised, L142) with
+// Dirichlet ends has the closed solution
+//     d_j = phi_j - phi_{j-1} = d_1 - S_{j-1},   S_m = sum_{i=1..m} rho_i,
+//     phi_j = phi_0 + j d_1 - T_{j-1},           T_m = sum_{i=1..m} S_i,
+//     d_1 = (phi_N - phi_0 + T_{N-1}) / N,
+// i.e. the Thomas recurrences (L142) summed in closed form, which turns the serial elimination into
+// two block-wide fp64 prefix sums.  E_j = (phi_{j-1} - phi_{j+1}) / 2 = -d_1 + (S_{j-1} + S_j) / 2.
+struct FieldArgs {
+    const double* rho;
+    double *phi, *E, *S, *Tt;
+    float* E32;
+    int Nc, nodes, bc;
+    double V0, omega_dt;
+    unsigned n_time;
+};
+
+__device__ double block_sum_d(double v) {
+    __shared__ double s_r[32];
+    __shared__ double s_out;
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    v = warp_sum_d(v);
+    if (lane == 0) s_r[wp] = v;
+    __syncthreads();
+    if (wp == 0) {
+        double t = lane < (blockDim.x >> 5) ? s_r[lane] : 0.0;
+        t = warp_sum_d(t);
+        if (lane == 0) s_out = t;
+    }
+    __syncthreads();
+    const double r = s_out;
+    __syncthreads();
+    return r;
+}
+
+// inclusive scan of n doubles, dst[i] = sum_{m<=i} src(m); thread-contiguous chunks.
+template <class F>
+__device__ void block_inclusive_scan_d(F src, double* dst, int n) {
+    __shared__ double s_w[32];
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5, nw = blockDim.x >> 5;
+    const int ch = (n + blockDim.x - 1) / blockDim.x;
+    const int b = tid * ch, e = min(b + ch, n);
+    double tot = 0.0;
+    for (int i = b; i < e; ++i) tot += src(i);
+    double inc = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        double t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_w[wp] = inc;
+    __syncthreads();
+    if (wp == 0) {
+        double t = lane < nw ? s_w[lane] : 0.0, ti = t;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            double u = __shfl_up_sync(0xffffffffu, ti, o);
+            if (lane >= o) ti += u;
+        }
+        s_w[lane] = ti - t;
+    }
+    __syncthreads();
+    double run = s_w[wp] + inc - tot;
+    for (int i = b; i < e; ++i) { run += src(i); dst[i] = run; }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(1024) k_field(FieldArgs a) {
+    const int N = a.Nc, tid = threadIdx.x;
+    double mean = 0.0;
+    if (a.bc == 1) {
+        double p = 0.0;
+        for (int i = tid; i < N; i += blockDim.x) p += a.rho[i];
+        mean = block_sum_d(p) / (double)N;
+    }
+    const double* rho = a.rho;
+    // S_j, j = 0..N-1 (S_0 = 0); T_j likewise
+    block_inclusive_scan_d([=](int i) { return i == 0 ? 0.0 : rho[i] - mean; }, a.S, N);
+    const double* S = a.S;
+    block_inclusive_scan_d([=](int i) { return S[i]; }, a.Tt, N);
+    const double phi0 = a.bc == 0 ? a.V0 * sin(a.omega_dt * (double)a.n_time) : 0.0;
+    const double phiN = 0.0;
+    const double d1 = (phiN - phi0 + a.Tt[N - 1]) / (double)N;
+    double psum = 0.0;
+    for (int j = tid; j < a.nodes; j += blockDim.x) {
+        double phi, E;
+        if (j == 0) {
+            phi = phi0;
+            E = a.bc == 0 ? -d1 - rho[0] : -d1 + 0.5 * S[N - 1];
+        } else if (j == N) {  // bounded only
+            phi = phiN;
+            E = -d1 + S[N - 1] + rho[N];
+        } else {
+            phi = phi0 + (double)j * d1 - a.Tt[j - 1];
+            E = -d1 + 0.5 * (S[j - 1] + S[j]);
+        }
+        a.phi[j] = phi;
+        a.E[j] = E;
+        a.E32[j] = (float)E;
+        psum += phi;
+    }
+    if (a.bc == 1) {  // report phi with its mean removed
+        const double pm = block_sum_d(psum) / (double)N;
+        for (int j = tid; j < N; j += blockDim.x) a.phi[j] -= pm;
+    }
+}
+
+// ---- moments (diagnostic, not on the step path) ------------------------------------------------------
+struct MomArgs {
+    const float *vx, *vy, *vz;
+    const DevState* st;
+    int s;
+    double* partial;  // [gridDim.x * 5]
+    ull* eedf;
+    int n_bins;
+    double E_max, c_eV;
+};
+
+__global__ void __launch_bounds__(256) k_moments(MomArgs a) {
+    const int n = a.st->sp[a.s].n_live;
+    double sx = 0, sy = 0, sz = 0, s2 = 0, s4 = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const double vx = a.vx[i], vy = a.vy[i], vz = a.vz[i];
+        const double g2 = (vx * vx + vy * vy) + vz * vz;
+        sx += vx; sy += vy; sz += vz; s2 += g2; s4 += g2 * g2;
+        if (a.eedf) {
+            const double En = a.c_eV * g2;
+            if (En < a.E_max) {
+                const int b = (int)(En / a.E_max * (double)a.n_bins);
+                if (b >= 0 && b < a.n_bins) atomicAdd(&a.eedf[b], 1ull);
+            }
+        }
+    }
+    sx = block_sum_d(sx); sy = block_sum_d(sy); sz = block_sum_d(sz);
+    s2 = block_sum_d(s2); s4 = block_sum_d(s4);
+    if (threadIdx.x == 0) {
+        double* p = a.partial + blockIdx.x * 5;
+        p[0] = sx; p[1] = sy; p[2] = sz; p[3] = s2; p[4] = s4;
+    }
+}
+
+// device-side validation of freshly loaded positions: x in [0, N_c)
+__global__ void k_validate(const float* x, int n, float fNc, DevState* st) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const float v = x[i];
+        if (!(v >= 0.0f && v < fNc)) atomicOr(&st->err, ERRBIT_BADLOAD);
+    }
+}

@@ -1,0 +1,406 @@
+// pic1d_sort.cuh -- fused gather + push + boundary with the fine sort.
+//
+// The paper sorts in place with per-cell slack and shared/global atomic counters (L166-186); here
+// the sort is a compact, STABLE counting sort in two passes over the particles, and the push is
+// recomputed in the second pass instead of being stored in between:
+//
+//   pass 1  k_push_count    read x, vx (8 B/particle); push; boundary; key; per-tile histogram in
+//                           shared memory; the tile's window [lo, hi] of counts goes to a pool
+//   scan    k_bin_scan      per sort cell k: exclusive prefix over tiles of count[t][k] (in place),
+//                           total -> hist[k]
+//           k_offsets_scan  exclusive scan of hist -> offsets[N_sc + 1]; prefix of absorbed counts
+//   pass 2  k_push_scatter  read x, vx, vy, vz (16 B); identical push; stable rank inside the tile
+//                           (warp match + shared counters, warps in order); write the four arrays to
+//                           offsets[k] + prefix[t][k] + rank (16 B)
+//
+// A tile is T consecutive source slots.  Because the source is sorted by last step's cell, a tile's
+// keys fall in a narrow window when particles move about one cell per step (Eq. 5); nothing
+// breaks when they do not (configs 2-4 electrons), the window just gets wider.
+#pragma once
+#include "pic1d_device.cuh"
+
+struct SortArgs {
+    const float *sx, *svx, *svy, *svz;  // source buffer
+    float *dx, *dvx, *dvy, *dvz;        // destination buffer
+    const float* E32;
+    DevState* st;
+    int s;
+    int *tile_lo, *tile_w, *tile_off, *tile_dead;  // per tile: window start, width, pool offset, absorbed
+    int *grp_lo, *grp_hi;                          // per tile group: union window
+    int* pool;
+    int pool_size;
+    int* hist;     // [n_sc]
+    int* offsets;  // [n_sc + 1]
+    int* keys_dbg; // optional, per source slot
+    unsigned* abs_list;  // optional ordered list of absorbed slots (ions, for secondary emission)
+    int abs_cap;
+    float kappa, fNc, inv_r;
+    int Nc, n_sc;
+};
+
+// ---- pass 1 -----------------------------------------------------------------------------------
+// V float4 loads per thread: tile T = NT * 4 * V slots.
+template <int BC, int V>
+__global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
+    extern __shared__ int s_hist[];  // n_sc counters, all zero between tiles
+    __shared__ int s_red[4][PIC1D_NWARP];
+    __shared__ int s_bc[3];
+    constexpr int T = PIC1D_NT * 4 * V;
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    DevSpecies& sp = a.st->sp[a.s];
+    const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
+    for (int i = tid; i < a.n_sc; i += PIC1D_NT) s_hist[i] = 0;
+    __syncthreads();
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int base = tile * T;
+        int keys[4 * V];
+        int lo = 0x7fffffff, hi = -1, ndl = 0, ndr = 0;
+        bool nonfinite = false;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const int idx = base + (v * PIC1D_NT + tid) * 4;
+            float4 X = make_float4(0.f, 0.f, 0.f, 0.f), VX = X;
+            if (idx < n_src) {
+                X = __ldcs(reinterpret_cast<const float4*>(a.sx + idx));
+                VX = __ldcs(reinterpret_cast<const float4*>(a.svx + idx));
+            }
+            float xs[4] = {X.x, X.y, X.z, X.w}, vs[4] = {VX.x, VX.y, VX.z, VX.w};
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int i = idx + c;
+                int key = -3;
+                if (i < n_src) {
+                    key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r);
+                    if (key >= 0) { lo = min(lo, key); hi = max(hi, key); }
+                    else if (key == -1) ++ndl;
+                    else { ++ndr; nonfinite |= (xs[c] != xs[c]); }
+                    if (a.keys_dbg) a.keys_dbg[i] = key >= 0 ? key : -1;
+                }
+                keys[v * 4 + c] = key;
+            }
+        }
+        lo = warp_min(lo); hi = warp_max(hi); ndl = warp_sum(ndl); ndr = warp_sum(ndr);
+        if (lane == 0) { s_red[0][wp] = lo; s_red[1][wp] = hi; s_red[2][wp] = ndl; s_red[3][wp] = ndr; }
+        if (nonfinite) atomicOr(&a.st->err, ERRBIT_NONFINITE);
+        __syncthreads();
+        if (tid == 0) {
+            int L = 0x7fffffff, H = -1, dl = 0, dr = 0;
+            for (int w = 0; w < PIC1D_NWARP; ++w) {
+                L = min(L, s_red[0][w]); H = max(H, s_red[1][w]); dl += s_red[2][w]; dr += s_red[3][w];
+            }
+            int w = H >= L ? H - L + 1 : 0;
+            int off = 0;
+            if (w > 0) {
+                off = atomicAdd(&sp.pool_used, w);
+                if (off + w > a.pool_size) { off = -1; atomicOr(&a.st->err, ERRBIT_WORKSPACE); }
+                atomicMin(&a.grp_lo[tile / PIC1D_GROUP], L);
+                atomicMax(&a.grp_hi[tile / PIC1D_GROUP], H);
+            } else {
+                L = 0;
+            }
+            a.tile_lo[tile] = L; a.tile_w[tile] = off >= 0 ? w : 0; a.tile_off[tile] = off;
+            a.tile_dead[tile] = dl + dr;
+            if (dl) atomicAdd(&sp.absorbed_left, (ull)dl);
+            if (dr) atomicAdd(&sp.absorbed_right, (ull)dr);
+            s_bc[0] = L; s_bc[1] = w; s_bc[2] = off;
+        }
+        __syncthreads();
+        lo = s_bc[0];
+        const int w = s_bc[1], off = s_bc[2];
+        // histogram: one shared atomic per run of equal keys; one per warp when the warp is uniform
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const int k0 = keys[v * 4], k1 = keys[v * 4 + 1], k2 = keys[v * 4 + 2], k3 = keys[v * 4 + 3];
+            const bool u4 = (k0 >= 0) & (k0 == k1) & (k1 == k2) & (k2 == k3);
+            const int kk = __shfl_sync(0xffffffffu, k0, 0);
+            if (__all_sync(0xffffffffu, u4 && k0 == kk)) {
+                if (lane == 0) atomicAdd(&s_hist[kk], 128);
+            } else {
+                int run = 1;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int k = keys[v * 4 + c];
+                    const bool last = (c == 3) || (keys[v * 4 + (c < 3 ? c + 1 : 3)] != k);
+                    if (last) { if (k >= 0) atomicAdd(&s_hist[k], run); run = 1; }
+                    else ++run;
+                }
+            }
+        }
+        __syncthreads();
+        for (int i = tid; i < w; i += PIC1D_NT) {
+            if (off >= 0) a.pool[off + i] = s_hist[lo + i];
+            s_hist[lo + i] = 0;
+        }
+        __syncthreads();
+    }
+}
+
+// ---- scan over tiles, per sort cell --------------------------------------------------------------
+// thread = one sort cell k.  pool[tile_off[t] + k - tile_lo[t]] becomes the number of particles of
+// tiles < t with key k (exclusive prefix); hist[k] the total.
+__global__ void __launch_bounds__(128) k_bin_scan(SortArgs a) {
+    const int k = blockIdx.x * 128 + threadIdx.x;
+    const int kb0 = blockIdx.x * 128, kb1 = min(kb0 + 127, a.n_sc - 1);
+    const int n_tiles = a.st->sp[a.s].n_tiles;
+    int run = 0;
+    const int n_groups = (n_tiles + PIC1D_GROUP - 1) / PIC1D_GROUP;
+    for (int g = 0; g < n_groups; ++g) {
+        const int glo = a.grp_lo[g], ghi = a.grp_hi[g];
+        if (ghi < kb0 || glo > kb1) continue;  // block-uniform
+        const int t1 = min((g + 1) * PIC1D_GROUP, n_tiles);
+        for (int t = g * PIC1D_GROUP; t < t1; ++t) {
+            const int lo = a.tile_lo[t], w = a.tile_w[t];
+            const unsigned r = (unsigned)(k - lo);
+            if (r < (unsigned)w) {
+                int* p = a.pool + a.tile_off[t] + r;
+                const int c = *p;
+                *p = run;
+                run += c;
+            }
+        }
+    }
+    if (k < a.n_sc) a.hist[k] = run;
+}
+
+// block-wide exclusive scan of src[0..n) into dst[0..n), returns the total; single block, any n.
+// dst may alias src.
+__device__ int block_exclusive_scan(const int* src, int* dst, int n, int carry_in) {
+    __shared__ int s_w[32];
+    __shared__ int s_carry;
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5, nw = blockDim.x >> 5;
+    if (tid == 0) s_carry = carry_in;
+    __syncthreads();
+    for (int base = 0; base < n; base += blockDim.x) {
+        const int i = base + tid;
+        const int v = i < n ? src[i] : 0;
+        int inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) s_w[wp] = inc;
+        __syncthreads();
+        if (wp == 0) {
+            int t = lane < nw ? s_w[lane] : 0;
+            int ti = t;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int u = __shfl_up_sync(0xffffffffu, ti, o);
+                if (lane >= o) ti += u;
+            }
+            s_w[lane] = ti - t;  // exclusive over warps
+            if (lane == 31) s_w[31] = ti - t;
+        }
+        __syncthreads();
+        const int carry = s_carry;
+        if (i < n) dst[i] = carry + s_w[wp] + inc - v;
+        __syncthreads();
+        if (tid == blockDim.x - 1) s_carry = carry + s_w[wp] + inc;
+        __syncthreads();
+    }
+    return s_carry;
+}
+
+// offsets[k] = #{key < k}; n_live = n_sorted = survivors; exclusive prefix of absorbed counts.
+__global__ void __launch_bounds__(1024) k_offsets_scan(SortArgs a) {
+    DevSpecies& sp = a.st->sp[a.s];
+    const int total = block_exclusive_scan(a.hist, a.offsets, a.n_sc, 0);
+    __syncthreads();
+    const int n_dead = block_exclusive_scan(a.tile_dead, a.tile_dead, sp.n_tiles, 0);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        a.offsets[a.n_sc] = total;
+        sp.n_live = total;
+        sp.n_sorted = total;
+        sp.n_dead = n_dead;
+    }
+}
+
+// ---- pass 2 -----------------------------------------------------------------------------------
+// ROWS rows of 32 consecutive slots per warp: tile T = NT * ROWS.
+template <int BC, int ROWS>
+__global__ void __launch_bounds__(PIC1D_NT) k_push_scatter(SortArgs a) {
+    extern __shared__ int s_cnt[];  // absolute destination counters, valid on the tile's window
+    __shared__ int s_dead;
+    constexpr int T = PIC1D_NT * ROWS;
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    const unsigned lt = lanemask_lt();
+    DevSpecies& sp = a.st->sp[a.s];
+    const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int lo = a.tile_lo[tile], w = a.tile_w[tile], off = a.tile_off[tile];
+        if (off < 0) continue;  // count pool exhausted (sticky ERR_WORKSPACE): drop the tile, write nothing
+        for (int i = tid; i < w; i += PIC1D_NT) s_cnt[lo + i] = a.offsets[lo + i] + a.pool[off + i];
+        if (tid == 0) s_dead = a.tile_dead[tile];
+        const int base = tile * T + wp * (ROWS * 32) + lane;
+        float x[ROWS], vx[ROWS], vy[ROWS], vz[ROWS];
+        int key[ROWS];
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r) {
+            const int i = base + r * 32;
+            key[r] = -3;
+            if (i < n_src) {
+                x[r] = __ldcs(a.sx + i); vx[r] = __ldcs(a.svx + i);
+                vy[r] = __ldcs(a.svy + i); vz[r] = __ldcs(a.svz + i);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r) {
+            const int i = base + r * 32;
+            if (i < n_src)
+                key[r] = push_particle<BC>(x[r], vx[r], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r);
+        }
+        __syncthreads();
+        // stable rank: warps take turns in slot order; inside a warp rows go in order and equal keys
+        // of one row are ranked by lane (match.any).  key[] is overwritten by the destination.
+        for (int turn = 0; turn < PIC1D_NWARP; ++turn) {
+            if (wp == turn) {
+#pragma unroll
+                for (int r = 0; r < ROWS; ++r) {
+                    const int mk = key[r] >= 0 ? key[r] : (key[r] == -3 ? -3 : -1);
+                    const int m0 = __shfl_sync(0xffffffffu, mk, 0);
+                    int dst;
+                    if (__all_sync(0xffffffffu, mk == m0 && mk >= 0)) {
+                        int b = 0;
+                        if (lane == 0) { b = s_cnt[mk]; s_cnt[mk] = b + 32; }
+                        dst = __shfl_sync(0xffffffffu, b, 0) + lane;
+                    } else {
+                        const unsigned peers = __match_any_sync(0xffffffffu, mk);
+                        const int leader = __ffs(peers) - 1;
+                        int b = 0;
+                        if (lane == leader) {
+                            if (mk >= 0) { b = s_cnt[mk]; s_cnt[mk] = b + __popc(peers); }
+                            else if (mk == -1) { b = s_dead; s_dead = b + __popc(peers); }
+                        }
+                        dst = __shfl_sync(0xffffffffu, b, leader) + __popc(peers & lt);
+                    }
+                    if (key[r] >= 0) key[r] = dst;
+                    else if (key[r] != -3) key[r] = -4 - 2 * dst - (key[r] == -2 ? 1 : 0);  // absorbed: rank, wall
+                    __syncwarp();
+                }
+            }
+            __syncthreads();
+        }
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r) {
+            const int d = key[r];
+            if (d >= 0) {
+                a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
+            } else if (d <= -4 && a.abs_list) {
+                const int e = -4 - d, rank = e >> 1, wall = e & 1;
+                if (rank < a.abs_cap) a.abs_list[rank] = (unsigned)(base + r * 32) | ((unsigned)wall << 31);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// ---- set up the sorts of one step ------------------------------------------------------------------
+// mode 0: initial sort after a load (nothing is pushed); mode 1: a regular step.
+__global__ void k_step_begin(DevState* st, int n_species, int mode, int T, int* grp_lo0, int* grp_hi0,
+                             int* grp_lo1, int* grp_hi1, int n_groups0, int n_groups1) {
+    const int tid = threadIdx.x + blockIdx.x * blockDim.x;
+    if (tid == 0) {
+        for (int s = 0; s < n_species; ++s) {
+            DevSpecies& sp = st->sp[s];
+            sp.n_push = mode ? sp.n_live : 0;
+            sp.n_src = sp.n_live;
+            sp.n_tiles = (sp.n_live + T - 1) / T;
+            sp.n_dead = 0;
+            sp.pool_used = 0;
+            sp.ticket = 0;
+        }
+        st->n_abs = 0;
+    }
+    for (int i = tid; i < n_groups0; i += blockDim.x * gridDim.x) { grp_lo0[i] = 0x7fffffff; grp_hi0[i] = -1; }
+    for (int i = tid; i < n_groups1; i += blockDim.x * gridDim.x) { grp_lo1[i] = 0x7fffffff; grp_hi1[i] = -1; }
+}
+
+// ---- secondary-electron emission at ion impact (L41; R19) --------------------------------
+struct SeeArgs {
+    DevState* st;
+    const unsigned* abs_list;
+    int abs_cap;
+    float *ex, *evx, *evy, *evz;  // electron SOURCE buffer of this step (injected after the survivors)
+    int cap_e;
+    int T;
+    float gamma, vth, fNc;
+    uint32_t k0, k1, step;
+};
+
+__global__ void __launch_bounds__(1024) k_see_emit(SeeArgs a) {
+    __shared__ int s_w[32];
+    __shared__ int s_run, s_tot;
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    DevState* st = a.st;
+    int n_abs = st->sp[1].n_dead;
+    if (n_abs > a.abs_cap) {
+        n_abs = a.abs_cap;
+        if (tid == 0) atomicOr(&st->err, ERRBIT_CAPACITY);
+    }
+    const int ne = st->sp[0].n_live;
+    const uint32_t step = a.step;
+    if (tid == 0) s_run = 0;
+    __syncthreads();
+    for (int base = 0; base < n_abs; base += 1024) {
+        const int i = base + tid;
+        bool emit = false;
+        uint32_t w[4];
+        unsigned slot = 0, wall = 0;
+        if (i < n_abs) {
+            const unsigned e = a.abs_list[i];
+            slot = e & 0x7fffffffu; wall = e >> 31;
+            philox4x32_10(slot, step, STREAM_SEE, 0u, a.k0, a.k1, w);
+            emit = u01(w[0]) < a.gamma;
+        }
+        const unsigned bal = __ballot_sync(0xffffffffu, emit);
+        if (lane == 0) s_w[wp] = __popc(bal);
+        __syncthreads();
+        if (wp == 0) {  // exclusive prefix over the 32 warps, chunk total
+            const int t = s_w[lane];
+            int ti = t;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int u = __shfl_up_sync(0xffffffffu, ti, o);
+                if (lane >= o) ti += u;
+            }
+            s_w[lane] = ti - t;
+            if (lane == 31) s_tot = ti;
+        }
+        __syncthreads();
+        const int idx = s_run + s_w[wp] + __popc(bal & lanemask_lt());  // ascending ion-slot order
+        if (emit) {
+            const int d = ne + idx;
+            if (d < a.cap_e) {
+                uint32_t w2[4];
+                philox4x32_10(slot, step, STREAM_SEE, 1u, a.k0, a.k1, w2);
+                const float u1 = u01(w[1]), u2 = u01(w[2]), u3 = u01(w[3]), u4 = u01(w2[0]);
+                float x, sgn;
+                if (wall == 0) { x = u1; sgn = 1.0f; }
+                else { x = fminf(__fsub_rn(a.fNc, __fsub_rn(1.0f, u1)), nextafterf(a.fNc, 0.0f)); sgn = -1.0f; }
+                const float rx = sqrtf(__fmul_rn(-2.0f, logf(__fsub_rn(1.0f, u2))));
+                const float rt = sqrtf(__fmul_rn(-2.0f, logf(__fsub_rn(1.0f, u3))));
+                const float ph = __fmul_rn(6.2831855f, u4);
+                a.ex[d] = x;
+                a.evx[d] = __fmul_rn(sgn, __fmul_rn(a.vth, rx));
+                a.evy[d] = __fmul_rn(a.vth, __fmul_rn(rt, cosf(ph)));
+                a.evz[d] = __fmul_rn(a.vth, __fmul_rn(rt, sinf(ph)));
+            }
+        }
+        __syncthreads();
+        if (tid == 0) s_run += s_tot;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        const int emitted = s_run;
+        const int room = a.cap_e - ne;
+        const int kept = emitted < room ? emitted : (room > 0 ? room : 0);
+        DevSpecies& se = st->sp[0];
+        se.n_src = ne + kept;
+        se.n_tiles = (se.n_src + a.T - 1) / a.T;
+        se.injected += (ull)kept;
+        if (emitted > kept) { se.dropped += (ull)(emitted - kept); atomicOr(&st->err, ERRBIT_CAPACITY); }
+        st->n_abs = n_abs;
+    }
+}

@@ -1,0 +1,208 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the oracle, element by element, on
+the same seeded inputs.  Bars (BASELINE.json north_star): keys / offsets / survivor counts / event
+masks bit-exact for a single step from identical state; x, v relative error <= 1e-6; rho relative
+L-inf <= 1e-9; 200-step density / potential / energy moments within 1 % relative L2."""
+import numpy as np
+import pytest
+
+from helpers import params, load, rel_linf, rel_l2
+from paper_1104_3998_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_V = 1e-6
+TOL_RHO = 1e-9
+TOL_FIELD = 1e-9
+
+
+def _mk(p):
+    from oracle import oracle as O
+    from paper_1104_3998_b200 import pic1d as G
+    p = dict(p)
+    p["flags"] = G.FLAG_CAPTURE
+    parts = W.make_particles(p)
+    o, g = O.Oracle(p), G.Pic1D(p)
+    load(o, parts)
+    load(g, parts)
+    return o, g, p
+
+
+def _vel_err(gv, ov):
+    gv = np.stack(gv, 1).astype(np.float64)
+    ov = np.stack(ov, 1).astype(np.float64)
+    nrm = np.maximum(np.linalg.norm(ov, axis=1), 1e-30)
+    return float(np.max(np.abs(gv - ov).max(1) / nrm)) if gv.size else 0.0
+
+
+def compare_state(o, g, p, check_keys=True, exact_x=True):
+    from oracle import oracle as O
+    from paper_1104_3998_b200 import pic1d as G
+    for s in range(p["n_species"]):
+        mo, mg = o.moments(s), g.moments(s)
+        for k in ("count", "n_sorted", "absorbed_left", "absorbed_right", "injected", "n_candidates",
+                  "n_events", "births", "dropped", "over_cap"):
+            assert mo[k] == mg[k], (s, k, mo[k], mg[k])
+        assert np.array_equal(o.debug_get(O.OFFSETS, s), g.debug_get(G.DBG_OFFSETS, s)), s
+        if check_keys:
+            assert np.array_equal(o.debug_get(O.KEYS, s), g.debug_get(G.DBG_KEYS, s)), s
+            assert np.array_equal(o.debug_get(O.MASK, s), g.debug_get(G.DBG_MASK, s)), s
+        ox, gx = o.debug_get(O.X, s), g.debug_get(G.DBG_X, s)
+        if exact_x:
+            assert np.array_equal(ox, gx), (s, np.nonzero(ox != gx)[0][:10])
+        else:
+            assert np.max(np.abs(ox.astype(np.float64) - gx) / np.maximum(np.abs(ox), 1.0)) <= TOL_V
+        ev = _vel_err([g.debug_get(w, s) for w in (G.DBG_VX, G.DBG_VY, G.DBG_VZ)],
+                      [o.debug_get(w, s) for w in (O.VX, O.VY, O.VZ)])
+        assert ev <= TOL_V, (s, ev)
+        assert rel_linf(g.debug_get(G.DBG_RHO_S, s), o.debug_get(O.RHO_S, s)) <= TOL_RHO
+        for k in ("sum_vx", "sum_vy", "sum_vz", "sum_v2", "sum_v4"):
+            scale = max(abs(mo["sum_v2"]), 1e-300) if k != "sum_v4" else max(abs(mo["sum_v4"]), 1e-300)
+            if k in ("sum_vx", "sum_vy", "sum_vz"):
+                scale = np.sqrt(max(mo["sum_v2"] * max(mo["count"], 1), 1e-300))
+            assert abs(mo[k] - mg[k]) <= 1e-5 * scale, (s, k, mo[k], mg[k])
+    ro, po, Eo = o.get_rho_phi_E()
+    rg, pg, Eg = g.get_rho_phi_E()
+    assert rel_linf(rg, ro) <= TOL_RHO
+    assert rel_linf(pg, po) <= TOL_FIELD, rel_linf(pg, po)
+    assert rel_linf(Eg, Eo) <= TOL_FIELD, rel_linf(Eg, Eo)
+
+
+CASES = {
+    "cfg0": dict(cfg_id=0),
+    "cfg0_ragged": dict(cfg_id=0, n_cells=100, ppc=83),
+    "cfg2_small": dict(cfg_id=2, n_cells=256, ppc=150),
+    "cfg2_ratio2": dict(cfg_id=2, n_cells=256, ppc=97, sort_ratio=2.0),
+    "cfg2_ratio05": dict(cfg_id=2, n_cells=128, ppc=120, sort_ratio=0.5),
+    "cfg2_ratio16": dict(cfg_id=2, n_cells=256, ppc=64, sort_ratio=16.0),
+    "cfg1_small": dict(cfg_id=1, ppc=40),
+    "cfg4_scaled": dict(cfg_id=4, n_cells=512, ppc=300),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_load_then_single_steps_from_identical_state(name):
+    """After the load and after each of a few steps (the oracle's E32 injected before every step so
+    both sides gather the identical field, R17) every discrete output is bit-exact."""
+    o, g, p = _mk(W.make_params(**CASES[name]))
+    from oracle import oracle as O
+    compare_state(o, g, p, check_keys=False)
+    for n in range(4):
+        g.set_E32(o.debug_get(O.E32))
+        assert o.step(1) == 0
+        g.step(1)
+        compare_state(o, g, p)
+    o.close(); g.close()
+
+
+def test_edge_cases_empty_and_single():
+    from oracle import oracle as O
+    from paper_1104_3998_b200 import pic1d as G
+    p = W.make_params(2, n_cells=64, ppc=4)
+    p["flags"] = G.FLAG_CAPTURE
+    z = np.zeros(0, np.float32)
+    one = (np.array([63.5], np.float32), np.array([1.0], np.float32), np.zeros(1, np.float32), np.zeros(1, np.float32))
+    for parts in ([(z, z, z, z), (z, z, z, z)], [(z, z, z, z), one], [one, (z, z, z, z)]):
+        o, g = O.Oracle(p), G.Pic1D(p)
+        load(o, parts); load(g, parts)
+        compare_state(o, g, p, check_keys=False)
+        for _ in range(2):
+            g.set_E32(o.debug_get(O.E32))
+            o.step(1); g.step(1)
+            compare_state(o, g, p)
+        o.close(); g.close()
+
+
+def test_all_ions_hit_walls_secondary_emission_order():
+    """every ion is absorbed in one step: stresses the ordered absorbed list and the SEE kernel"""
+    from oracle import oracle as O
+    from paper_1104_3998_b200 import pic1d as G
+    n = 30000
+    p = W.make_params(2, n_cells=64, ppc=1, capacity_factor=1500, mcc=False)
+    p["flags"] = G.FLAG_CAPTURE
+    xi = np.where(np.arange(n) % 3 == 0, 0.5, 63.5).astype(np.float32)
+    vi = np.where(np.arange(n) % 3 == 0, -1.0, 1.0).astype(np.float32)
+    rng = np.random.default_rng(2)
+    xe = (rng.random(5000, dtype=np.float32) * 64).astype(np.float32)
+    ve = rng.normal(size=5000).astype(np.float32)
+    parts = [(xe, ve, 0 * xe, 0 * xe), (xi, vi, 0 * xi, 0 * xi)]
+    o, g = O.Oracle(p), G.Pic1D(p)
+    load(o, parts); load(g, parts)
+    zero = np.zeros(65, np.float32)
+    o.set_E32(zero); g.set_E32(zero)
+    o.step(1); g.step(1)
+    compare_state(o, g, p)
+    assert g.moments(0)["injected"] > 2000 and g.moments(1)["count"] == 0
+    o.close(); g.close()
+
+
+def test_capacity_overflow_is_sticky_and_safe():
+    from paper_1104_3998_b200 import pic1d as G
+    p = W.make_params(2, n_cells=64, ppc=64, capacity_factor=1.0)
+    for s in range(2):
+        p["species"][s]["capacity"] = 4096
+    parts = W.make_particles(p)
+    g = G.Pic1D(p)
+    load(g, parts)
+    with pytest.raises(G.Pic1DError) as e:
+        g.load_particles(0, *[np.zeros(5000, np.float32)] * 4)
+    assert e.value.code == G.ERR_CAPACITY
+    g.close()
+
+
+def test_bad_positions_rejected():
+    from paper_1104_3998_b200 import pic1d as G
+    p = W.make_params(0)
+    parts = W.make_particles(p)
+    parts[0][0][17] = 500.0
+    g = G.Pic1D(p)
+    load(g, parts)
+    g.get_rho_phi_E()
+    assert g.sticky == G.ERR_ARG
+    g.close()
+
+
+@pytest.mark.parametrize("name,steps", [("cfg0", 100), ("cfg2_small", 200)])
+def test_long_run_moments_within_1pct(name, steps):
+    """free-running (no field injection): time-averaged density, potential and energy moments"""
+    o, g, p = _mk(W.make_params(**CASES[name]))
+    acc = {k: 0.0 for k in ("ne_o", "ne_g", "ni_o", "ni_g", "phi_o", "phi_g")}
+    en = []
+    for n in range(steps):
+        assert o.step(1) == 0
+        g.step(1)
+        if n % 10 == 9 or n == steps - 1:
+            mo, mg = [o.moments(s) for s in range(2)], [g.moments(s) for s in range(2)]
+            acc["ne_o"] = acc["ne_o"] + mo[0]["density"]; acc["ne_g"] = acc["ne_g"] + mg[0]["density"]
+            acc["ni_o"] = acc["ni_o"] + mo[1]["density"]; acc["ni_g"] = acc["ni_g"] + mg[1]["density"]
+            acc["phi_o"] = acc["phi_o"] + o.get_rho_phi_E()[1]; acc["phi_g"] = acc["phi_g"] + g.get_rho_phi_E()[1]
+            for s in range(2):
+                en.append((mo[s]["sum_v2"] / mo[s]["count"], mg[s]["sum_v2"] / mg[s]["count"],
+                           mo[s]["sum_v4"] / mo[s]["count"], mg[s]["sum_v4"] / mg[s]["count"]))
+    assert rel_l2(acc["ne_g"], acc["ne_o"]) <= 0.01
+    assert rel_l2(acc["ni_g"], acc["ni_o"]) <= 0.01
+    assert rel_l2(acc["phi_g"], acc["phi_o"]) <= 0.01
+    en = np.array(en)
+    assert np.all(np.abs(en[:, 1] / en[:, 0] - 1) <= 0.01)
+    assert np.all(np.abs(en[:, 3] / en[:, 2] - 1) <= 0.02)
+    for s in range(2):
+        assert abs(g.moments(s)["count"] / o.moments(s)["count"] - 1) <= 0.01
+    o.close(); g.close()
+
+
+def test_cold_plasma_frequency_on_gpu():
+    """config 1 (scaled ppc) on the GPU alone: omega within 1 % of omega_p (closed form)"""
+    from paper_1104_3998_b200 import pic1d as G
+    p = W.make_params(1, ppc=200)
+    g = G.Pic1D(p)
+    load(g, W.make_particles(p))
+    k = 2 * np.pi * np.arange(512) / 512
+    amp = []
+    for n in range(600):
+        g.step(1)
+        amp.append(2 * np.mean(g.get_rho_phi_E()[2] * np.sin(k)))
+    amp = np.array(amp)
+    zc = np.nonzero(amp[:-1] * amp[1:] < 0)[0]
+    tz = zc + amp[zc] / (amp[zc] - amp[zc + 1])
+    w = np.pi / np.mean(np.diff(tz))
+    assert abs(w / 0.1 - 1) < 0.01
+    g.close()
