@@ -1,0 +1,324 @@
+#!/usr/bin/env python
+"""bench.py -- particle-steps/s of the full PIC/MCC cycle (BASELINE.json metric) on synthetic input.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl reference]
+
+A "step" is one pass of the whole hot path (push, boundary, fine sort, deposit, Poisson + E, MCC)
+over all particles of the workload.  N = 1 runs BASELINE.json config 4 (16384 cells, 4000
+particles per cell per species, ~1.31e8 particles, 2.1 GB of fp32 SoA state).  N > 1: the path is
+single-GPU by construction (replicas only), so every rank runs an
+independent replica and `value` is the sum over ranks.  One JSON line on stdout (rank 0).
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1104_3998_b200 import workloads as W  # noqa: E402
+
+METRIC = "particle-steps/sec (full PIC/MCC cycle)"
+UNIT = "particle-steps/s"
+
+
+def measured_peak():
+    f = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(f):
+        try:
+            return float(json.load(open(f))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def workload_name(p):
+    return "config[%d] %s: %d cells x %d ppc x %d species, r=%g%s" % (
+        p["cfg_id"], p["name"], p["n_cells"], p["ppc"], p["n_species"], p["sort_ratio"],
+        " (Courant twin)" if p["courant"] else "")
+
+
+# ---------------------------------------------------------------------------------------------
+class ClockSampler(threading.Thread):
+    """samples SM clock and throttle reasons with NVML while the timed region runs"""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag, self.max_mhz = index, [], set(), False, None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                     nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                     nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                     nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+            while not self.stop_flag:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                time.sleep(0.01)
+        except Exception as e:  # NVML missing: report it, do not fail the bench
+            self.reasons.add("nvml_unavailable:%s" % type(e).__name__)
+
+    def result(self):
+        self.stop_flag = True
+        self.join(timeout=2)
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------
+def run_oracle_sample(p_full, steps, warmup):
+    """The oracle as it stands, one thread, on a bounded sample of the workload: same grid, same
+    constants, ppc reduced so that the run takes seconds."""
+    from oracle import oracle as O
+    ppc = max(8, min(p_full["ppc"], 100))
+    p = W.make_params(p_full["cfg_id"], n_cells=p_full["n_cells"], ppc=ppc, sort_ratio=p_full["sort_ratio"],
+                      courant=p_full["courant"])
+    parts = W.make_particles(p)
+    o = O.Oracle(p)
+    for s, a in enumerate(parts):
+        o.load_particles(s, *a)
+    o.step(warmup)
+    n0 = sum(o.moments(s)["count"] for s in range(p["n_species"]))
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    n1 = sum(o.moments(s)["count"] for s in range(p["n_species"]))
+    o.close()
+    value = 0.5 * (n0 + n1) * steps / dt
+    sample = "%s at ppc=%d (%d particles; the timed workload has ppc=%d), %d steps after %d warm-up" % (
+        p["name"], ppc, n0, p_full["ppc"], steps, warmup)
+    return value, dt / steps * 1e3, sample
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def reference_arm(args, p):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps = max(1, min(args.steps, 10))
+    value, ms, sample = run_oracle_sample(p, steps, min(args.warmup, 2))
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(p), "timed": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "host_cpu": cpu_model(), "nproc": os.cpu_count()},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ---------------------------------------------------------------------------------------------
+def algorithmic_bytes(name, n_src, n_out, n_sorted, cand_frac, coll_frac):
+    """SURVEY 8(d)-D4 / DESIGN.md: bytes the method must move, per launch"""
+    if name == "push_count":
+        return 8.0 * n_src                       # read x, vx
+    if name == "push_scatter":
+        return 16.0 * n_src + 16.0 * n_out       # read 4 arrays, write 4 arrays
+    if name == "deposit":
+        return 4.0 * n_sorted                    # read sorted x
+    if name == "mcc":
+        rd = 12.0 * (1.0 - (1.0 - cand_frac) ** 8)
+        wr = 12.0 * (1.0 - (1.0 - coll_frac) ** 8)
+        return (rd + wr) * n_sorted
+    return 0.0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=60)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--ppc", type=int, default=None)
+    ap.add_argument("--n-cells", type=int, default=None)
+    ap.add_argument("--sort-ratio", type=float, default=1.0)
+    ap.add_argument("--courant", action="store_true")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    assert args.warmup >= 3 or args.impl == "reference", "timing rule: at least 3 warm-up steps"
+
+    p = W.make_params(args.config, n_cells=args.n_cells, ppc=args.ppc, sort_ratio=args.sort_ratio,
+                      courant=args.courant)
+    if args.impl == "reference":
+        return reference_arm(args, p)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1104_3998_b200 import pic1d as G
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    # replicas only: rank r runs its own discharge (seed + r) on its own GPU
+    p["seed"] = p["seed"] + rank
+    parts = W.make_particles(p)
+    pinned = [[torch.from_numpy(a).pin_memory() for a in sp] for sp in parts]
+    sim = G.Pic1D(p, device=dev)
+    for s, sp in enumerate(pinned):
+        sim.load_particles(s, *[t.numpy() for t in sp])
+    ns = p["n_species"]
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def live():
+        return [sim.moments(s) for s in range(ns)]
+
+    sim.step(args.warmup)
+    barrier()
+    m0 = live()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    l0 = sim.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(sim.stream)
+    sim.step(args.steps)
+    e1.record(sim.stream)
+    barrier()
+    clocks = sampler.result()
+    ms = e0.elapsed_time(e1)
+    launches = sim.launch_count - l0
+    m1 = live()
+    n_mean = 0.5 * (sum(m["count"] for m in m0) + sum(m["count"] for m in m1))
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    tot = torch.tensor([n_mean], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    ms_max, n_total = float(t.item()), float(tot.item())
+    value = n_total * args.steps / (ms_max * 1e-3)
+
+    # per-kernel times (CUDA events between the kernels on the library's stream), same state
+    ksteps = max(3, min(args.steps, 20))
+    agg = {}
+    step_ms_timed = 0.0
+    mk0 = live()
+    for _ in range(ksteps):
+        for name, s, kms in sim.step_timed():
+            a = agg.setdefault((name, s), [0.0, 0])
+            a[0] += kms
+            a[1] += 1
+            step_ms_timed += kms
+    mk1 = live()
+    step_ms_timed /= ksteps
+    peak, peak_src = measured_peak()
+    kern = []
+    dom = None
+    for (name, s), (tms, cnt) in sorted(agg.items(), key=lambda kv: -kv[1][0]):
+        avg = tms / cnt
+        row = {"kernel": name, "species": s, "ms": avg, "share": tms / ksteps / step_ms_timed}
+        if s >= 0:
+            n_in = 0.5 * (mk0[s]["count"] + mk1[s]["count"])
+            n_out = 0.5 * (mk0[s]["n_sorted"] + mk1[s]["n_sorted"])
+            d = {k: mk1[s][k] - mk0[s][k] for k in ("n_candidates",)}
+            dev_ev = [mk1[s]["n_events"][k] - mk0[s]["n_events"][k] for k in range(4)]
+            cand = d["n_candidates"] / max(ksteps * n_out, 1)
+            coll = sum(dev_ev[1:]) / max(ksteps * n_out, 1)
+            b = algorithmic_bytes(name, n_in, n_out, n_out, cand, coll)
+            if b > 0:
+                row["alg_bytes"] = b
+                row["alg_GBps"] = b / (avg * 1e-3) / 1e9
+                row["frac_of_peak"] = row["alg_GBps"] / peak
+        kern.append(row)
+        if dom is None and "alg_GBps" in row:
+            dom = row
+    step_bytes = sum(r.get("alg_bytes", 0.0) for r in kern)
+    roofline = {"bound": "hbm", "kernel": "%s[s=%d]" % (dom["kernel"], dom["species"]),
+                "achieved": dom["alg_GBps"], "peak": peak, "unit": "GB/s", "frac": dom["alg_GBps"] / peak,
+                "traffic": None, "peak_source": peak_src, "alg_bytes_per_launch": dom["alg_bytes"],
+                "kernel_ms": dom["ms"],
+                "step": {"alg_bytes": step_bytes, "achieved": step_bytes / (ms_max / args.steps * 1e-3) / 1e9,
+                         "frac": step_bytes / (ms_max / args.steps * 1e-3) / 1e9 / peak,
+                         "frac_of_8TBps": step_bytes / (ms_max / args.steps * 1e-3) / 1e9 / 8000.0}}
+    tf = os.path.join(ROOT, "profiles", "traffic.txt")
+    if os.path.exists(tf):
+        for line in open(tf):
+            w = line.split()
+            if len(w) >= 2 and w[0] == roofline["kernel"]:
+                roofline["traffic"] = float(w[1])
+
+    # end to end through the public API with HOST buffers: every step re-loads the particles from
+    # pinned host memory (H2D), advances one step, and reads rho/phi/E back (D2H)
+    h2d = sum(t_.numel() * 4 for sp in pinned for t_ in sp)
+    out = [torch.empty(sim.n_nodes, dtype=torch.float64).pin_memory().numpy() for _ in range(3)]
+    d2h = 3 * sim.n_nodes * 8
+    n_e2e = sum(sp[0].numel() for sp in pinned)
+
+    def e2e_step():
+        for s, sp in enumerate(pinned):
+            sim.load_particles(s, *[t_.numpy() for t_ in sp])
+        sim.step(1)
+        sim.get_rho_phi_E(out)
+
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = n_e2e * world * args.e2e_steps / float(te.item())
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, cms, sample = run_oracle_sample(p, 5, 1)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+               "ms_per_step": cms, "host_cpu": cpu_model(), "nproc": os.cpu_count()}
+
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(p), "particles_per_gpu": n_mean,
+                       "l2": "inputs larger than L2 (%.2f GB of particle state per GPU)" % (n_mean * 16 / 1e9),
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "capture_masks": False, "tile": None},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": args.e2e_steps, "note": "load_particles(host) + step(1) + get_rho_phi_E(host) per step"},
+            "roofline": roofline, "cpu_baseline": cpu,
+            "kernels": kern, "ms_per_step_with_kernel_events": step_ms_timed}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -34,9 +34,11 @@ extern "C" {
 #define PIC1D_ERR_CUDA (-3)      /* a CUDA call failed; see pic1d_last_cuda_error */
 #define PIC1D_ERR_NONFINITE (-4) /* sticky: a NaN position was seen (treated as absorbed) */
 #define PIC1D_ERR_WORKSPACE (-5) /* workspace too small / sort bookkeeping pool exhausted (sticky) */
+#define PIC1D_ERR_ORDER (-6)     /* sticky: the rank self-check of PIC1D_FLAG_VERIFY_ORDER failed */
 
 /* flags */
 #define PIC1D_FLAG_CAPTURE 1u /* keep per-slot pre-sort keys and MCC event masks for pic1d_debug_get */
+#define PIC1D_FLAG_VERIFY_ORDER 2u /* re-check every in-tile rank of the scatter with match.any (slow) */
 
 typedef struct pic1d pic1d_t; /* opaque */
 

@@ -59,8 +59,8 @@ struct pic1d {
     bool ready;
     int64_t launches;
     cudaError_t last_err;
-    int grid_count, grid_scatter;
-    size_t smem_sort;
+    int grid_count, grid_scatter, WA;
+    size_t smem_sort, smem_scatter;
     bool timing;
     std::vector<TimeMark> marks;
     std::vector<cudaEvent_t> ev_pool;
@@ -203,6 +203,7 @@ SortArgs sort_args(pic1d* h, int s) {
     a.abs_cap = h->abs_cap;
     a.kappa = (float)h->cfg.sp[s].kappa;
     a.fNc = (float)h->cfg.n_cells; a.inv_r = h->inv_r; a.Nc = h->cfg.n_cells; a.n_sc = h->n_sc;
+    a.shift = 0; a.WA = h->WA; a.verify = (h->cfg.flags & PIC1D_FLAG_VERIFY_ORDER) ? 1 : 0;
     return a;
 }
 
@@ -217,9 +218,9 @@ void launch_count(pic1d* h, const SortArgs& a, int grid) {
 template <int BC>
 void launch_scatter(pic1d* h, const SortArgs& a, int grid) {
     switch (h->T) {
-        case 4096: k_push_scatter<BC, 16><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
-        case 2048: k_push_scatter<BC, 8><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
-        default: k_push_scatter<BC, 4><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
+        case 4096: k_push_scatter<BC, 16><<<grid, PIC1D_NT, h->smem_scatter, h->stream>>>(a); break;
+        case 2048: k_push_scatter<BC, 8><<<grid, PIC1D_NT, h->smem_scatter, h->stream>>>(a); break;
+        default: k_push_scatter<BC, 4><<<grid, PIC1D_NT, h->smem_scatter, h->stream>>>(a); break;
     }
 }
 
@@ -234,28 +235,35 @@ int occupancy_grid(pic1d* h, K kernel, size_t smem) {
 void setup_launch(pic1d* h) {
     const size_t smem = (size_t)h->n_sc * sizeof(int);
     h->smem_sort = smem;
+    h->WA = std::min(h->n_sc + 1, 2048);
+    const size_t sm2 = (size_t)h->WA * 5 * sizeof(unsigned);
+    h->smem_scatter = sm2;
     int gc, gs;
     if (h->cfg.bc == 1) {
-        if (h->T == 4096) { gc = occupancy_grid(h, k_push_count<1, 4>, smem); gs = occupancy_grid(h, k_push_scatter<1, 16>, smem); }
-        else if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<1, 2>, smem); gs = occupancy_grid(h, k_push_scatter<1, 8>, smem); }
-        else { gc = occupancy_grid(h, k_push_count<1, 1>, smem); gs = occupancy_grid(h, k_push_scatter<1, 4>, smem); }
+        if (h->T == 4096) { gc = occupancy_grid(h, k_push_count<1, 4>, smem); gs = occupancy_grid(h, k_push_scatter<1, 16>, sm2); }
+        else if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<1, 2>, smem); gs = occupancy_grid(h, k_push_scatter<1, 8>, sm2); }
+        else { gc = occupancy_grid(h, k_push_count<1, 1>, smem); gs = occupancy_grid(h, k_push_scatter<1, 4>, sm2); }
     } else {
-        if (h->T == 4096) { gc = occupancy_grid(h, k_push_count<0, 4>, smem); gs = occupancy_grid(h, k_push_scatter<0, 16>, smem); }
-        else if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<0, 2>, smem); gs = occupancy_grid(h, k_push_scatter<0, 8>, smem); }
-        else { gc = occupancy_grid(h, k_push_count<0, 1>, smem); gs = occupancy_grid(h, k_push_scatter<0, 4>, smem); }
+        if (h->T == 4096) { gc = occupancy_grid(h, k_push_count<0, 4>, smem); gs = occupancy_grid(h, k_push_scatter<0, 16>, sm2); }
+        else if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<0, 2>, smem); gs = occupancy_grid(h, k_push_scatter<0, 8>, sm2); }
+        else { gc = occupancy_grid(h, k_push_count<0, 1>, smem); gs = occupancy_grid(h, k_push_scatter<0, 4>, sm2); }
     }
     h->grid_count = gc;
     h->grid_scatter = gs;
 }
 
 // fine sort of species s (mode 0: no push)
-void enqueue_sort(pic1d* h, int s) {
+void enqueue_sort(pic1d* h, int s, int shift = 0) {
     SpeciesHost& p = h->sp[s];
     SortArgs a = sort_args(h, s);
+    if (shift > 0) {  // coarse pass of an unsorted load: sort by (sort cell >> shift)
+        a.shift = shift;
+        a.n_sc = ((h->n_sc - 1) >> shift) + 1;
+    }
     const int gc = std::min(h->grid_count, p.n_tiles_max), gs = std::min(h->grid_scatter, p.n_tiles_max);
     if (h->cfg.bc == 1) launch_count<1>(h, a, gc); else launch_count<0>(h, a, gc);
     mark(h, "push_count", s);
-    k_bin_scan<<<(h->n_sc + 127) / 128, 128, 0, h->stream>>>(a);
+    k_bin_scan<<<(a.n_sc + 127) / 128, 128, 0, h->stream>>>(a);
     mark(h, "bin_scan", s);
     k_offsets_scan<<<1, 1024, 0, h->stream>>>(a);
     mark(h, "offsets_scan", s);
@@ -353,6 +361,7 @@ int sticky_code(unsigned err) {
     if (err & ERRBIT_CAPACITY) return PIC1D_ERR_CAPACITY;
     if (err & ERRBIT_WORKSPACE) return PIC1D_ERR_WORKSPACE;
     if (err & ERRBIT_BADLOAD) return PIC1D_ERR_ARG;
+    if (err & ERRBIT_ORDER) return PIC1D_ERR_ORDER;
     return PIC1D_OK;
 }
 
@@ -452,6 +461,17 @@ int pic1d_load_particles(pic1d_t* h, int s, int64_t n, const float* x, const flo
         SpeciesHost& pq = h->sp[q];
         cudaMemsetAsync(pq.desc, 0, sizeof(ull) * pq.n_mcc_tiles, h->stream);
         if (pq.mask) cudaMemsetAsync(pq.mask, 0, pq.capacity, h->stream);
+    }
+    // An unsorted load has full-width tile windows.  If the count pool cannot hold them, sort first
+    // by a coarse key (sort cell >> shift), then by the sort cell: two stable passes = one stable sort.
+    int shift = 0;
+    for (int q = 0; q < h->cfg.n_species; ++q) {
+        const SpeciesHost& pq = h->sp[q];
+        while ((int64_t)(((h->n_sc - 1) >> shift) + 1) * pq.n_tiles_max > pq.pool_size) ++shift;
+    }
+    if (shift > 0) {
+        enqueue_begin(h, 0);
+        for (int q = h->cfg.n_species - 1; q >= 0; --q) enqueue_sort(h, q, shift);
     }
     enqueue_begin(h, 0);
     for (int q = h->cfg.n_species - 1; q >= 0; --q) enqueue_sort(h, q);

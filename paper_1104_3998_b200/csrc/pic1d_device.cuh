@@ -20,6 +20,7 @@
 #define ERRBIT_NONFINITE 2u
 #define ERRBIT_WORKSPACE 4u
 #define ERRBIT_BADLOAD 8u
+#define ERRBIT_ORDER 16u  // rank self-check failed (PIC1D_FLAG_VERIFY_ORDER)
 
 typedef unsigned long long ull;
 
@@ -92,7 +93,7 @@ __device__ __forceinline__ int warp_sum(int v) {
 template <int BC>
 __device__ __forceinline__ int push_particle(float& x, float& vx, bool do_push,
                                              const float* __restrict__ E32, float kappa, int Nc,
-                                             float fNc, float inv_r) {
+                                             float fNc, float inv_r, int shift) {
     if (do_push) {
         int j = (int)x;  // "single type casting operation", L87
         float f = __fsub_rn(x, (float)j);
@@ -110,5 +111,5 @@ __device__ __forceinline__ int push_particle(float& x, float& vx, bool do_push,
     } else if (!(x >= 0.0f && x < fNc)) {
         return x < 0.0f ? -1 : -2;
     }
-    return (int)__fmul_rn(x, inv_r);
+    return ((int)__fmul_rn(x, inv_r)) >> shift;  // shift > 0 only in the coarse pass of a load
 }

@@ -106,8 +106,8 @@ __global__ void k_rho_combine(CombineArgs a) {
     double r = a.background;
     for (int s = 0; s < a.n_species; ++s) {
         double v = j < a.Nc ? a.part[s][j] : 0.0;  // part is indexed by node because blocks are G-aligned
-        if (j > 0 && j % a.G == 0) v += a.side[s][j / a.G - 1];
         if (j == a.Nc) v += a.side[s][nb - 1];               // bounded: right wall node
+        else if (j > 0 && j % a.G == 0) v += a.side[s][j / a.G - 1];
         if (a.bc == 1 && j == 0) v += a.side[s][nb - 1];     // periodic: node N_c == node 0
         a.rho_s[s][j] = v;
         r += (double)a.sign[s] * v;

