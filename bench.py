@@ -159,6 +159,8 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profile", action="store_true",
+                    help="timed region only (no per-kernel pass, e2e or CPU baseline): the command ncu wraps")
     args = ap.parse_args()
     assert args.warmup >= 3 or args.impl == "reference", "timing rule: at least 3 warm-up steps"
 
@@ -221,6 +223,16 @@ def main():
         dist.all_reduce(tot, op=dist.ReduceOp.SUM)
     ms_max, n_total = float(t.item()), float(tot.item())
     value = n_total * args.steps / (ms_max * 1e-3)
+
+    if args.profile:
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
+                              "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps,
+                              "config": {"workload": workload_name(p)}, "gpu_launches": launches,
+                              "profile_only": True}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
 
     # per-kernel times (CUDA events between the kernels on the library's stream), same state
     ksteps = max(3, min(args.steps, 20))

@@ -114,7 +114,7 @@ size_t layout(pic1d* h, char* base) {
     h->inv_r = (float)c.sort_inv_ratio;
     int64_t cap_max = 0;
     for (int s = 0; s < c.n_species; ++s) cap_max = std::max<int64_t>(cap_max, c.sp[s].capacity);
-    h->T = cap_max >= 4096ll * 592 ? 4096 : (cap_max >= 2048ll * 592 ? 2048 : 1024);
+    h->T = cap_max >= 2048ll * 592 ? 2048 : 1024;
     const int rr = c.sort_inv_ratio < 1.0 ? (int)std::llround(1.0 / c.sort_inv_ratio) : 1;
     const int ppc_est = (int)std::max<int64_t>(1, cap_max / c.n_cells);
     h->G = std::min(2048, std::max(rr, pow2_floor(std::max(1, 4096 / ppc_est))));
@@ -209,19 +209,13 @@ SortArgs sort_args(pic1d* h, int s) {
 
 template <int BC>
 void launch_count(pic1d* h, const SortArgs& a, int grid) {
-    switch (h->T) {
-        case 4096: k_push_count<BC, 4><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
-        case 2048: k_push_count<BC, 2><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
-        default: k_push_count<BC, 1><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a); break;
-    }
+    if (h->T == 2048) k_push_count<BC, 2><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a);
+    else k_push_count<BC, 1><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a);
 }
 template <int BC>
 void launch_scatter(pic1d* h, const SortArgs& a, int grid) {
-    switch (h->T) {
-        case 4096: k_push_scatter<BC, 16><<<grid, PIC1D_NT, h->smem_scatter, h->stream>>>(a); break;
-        case 2048: k_push_scatter<BC, 8><<<grid, PIC1D_NT, h->smem_scatter, h->stream>>>(a); break;
-        default: k_push_scatter<BC, 4><<<grid, PIC1D_NT, h->smem_scatter, h->stream>>>(a); break;
-    }
+    if (h->T == 2048) k_push_scatter<BC, 8><<<grid, PIC1D_NT, h->smem_scatter, h->stream>>>(a);
+    else k_push_scatter<BC, 4><<<grid, PIC1D_NT, h->smem_scatter, h->stream>>>(a);
 }
 
 template <class K>
@@ -233,19 +227,17 @@ int occupancy_grid(pic1d* h, K kernel, size_t smem) {
 }
 
 void setup_launch(pic1d* h) {
-    const size_t smem = (size_t)h->n_sc * sizeof(int);
-    h->smem_sort = smem;
     h->WA = std::min(h->n_sc + 1, 2048);
+    const size_t smem = (size_t)h->WA * sizeof(int);
+    h->smem_sort = smem;
     const size_t sm2 = (size_t)h->WA * 5 * sizeof(unsigned);
     h->smem_scatter = sm2;
     int gc, gs;
     if (h->cfg.bc == 1) {
-        if (h->T == 4096) { gc = occupancy_grid(h, k_push_count<1, 4>, smem); gs = occupancy_grid(h, k_push_scatter<1, 16>, sm2); }
-        else if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<1, 2>, smem); gs = occupancy_grid(h, k_push_scatter<1, 8>, sm2); }
+        if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<1, 2>, smem); gs = occupancy_grid(h, k_push_scatter<1, 8>, sm2); }
         else { gc = occupancy_grid(h, k_push_count<1, 1>, smem); gs = occupancy_grid(h, k_push_scatter<1, 4>, sm2); }
     } else {
-        if (h->T == 4096) { gc = occupancy_grid(h, k_push_count<0, 4>, smem); gs = occupancy_grid(h, k_push_scatter<0, 16>, sm2); }
-        else if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<0, 2>, smem); gs = occupancy_grid(h, k_push_scatter<0, 8>, sm2); }
+        if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<0, 2>, smem); gs = occupancy_grid(h, k_push_scatter<0, 8>, sm2); }
         else { gc = occupancy_grid(h, k_push_count<0, 1>, smem); gs = occupancy_grid(h, k_push_scatter<0, 4>, sm2); }
     }
     h->grid_count = gc;
@@ -263,7 +255,7 @@ void enqueue_sort(pic1d* h, int s, int shift = 0) {
     const int gc = std::min(h->grid_count, p.n_tiles_max), gs = std::min(h->grid_scatter, p.n_tiles_max);
     if (h->cfg.bc == 1) launch_count<1>(h, a, gc); else launch_count<0>(h, a, gc);
     mark(h, "push_count", s);
-    k_bin_scan<<<(a.n_sc + 127) / 128, 128, 0, h->stream>>>(a);
+    k_bin_scan<<<(a.n_sc + 31) / 32, BINSCAN_NW * 32, 0, h->stream>>>(a);
     mark(h, "bin_scan", s);
     k_offsets_scan<<<1, 1024, 0, h->stream>>>(a);
     mark(h, "offsets_scan", s);

@@ -42,52 +42,79 @@ struct SortArgs {
 };
 
 // ---- pass 1 -----------------------------------------------------------------------------------
-// V float4 loads per thread: tile T = NT * 4 * V slots.
+// V float4 loads per thread: tile T = NT * 4 * V slots.  The tile's histogram lives in a shared
+// window of WA counters relative to the tile's lowest key; wider windows are counted WA bins at a time.
 template <int BC, int V>
 __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
-    extern __shared__ int s_hist[];  // n_sc counters, all zero between tiles
+    extern __shared__ int s_hist[];  // WA counters, all zero between tiles
     __shared__ int s_red[4][PIC1D_NWARP];
     __shared__ int s_bc[3];
     constexpr int T = PIC1D_NT * 4 * V;
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    const int WA = a.WA;
     DevSpecies& sp = a.st->sp[a.s];
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
-    for (int i = tid; i < a.n_sc; i += PIC1D_NT) s_hist[i] = 0;
+    for (int i = tid; i < WA; i += PIC1D_NT) s_hist[i] = 0;
     __syncthreads();
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const int base = tile * T;
         int keys[4 * V];
         int lo = 0x7fffffff, hi = -1, ndl = 0, ndr = 0;
         bool nonfinite = false;
+        const bool full = base + T <= n_push && a.keys_dbg == nullptr;  // block-uniform fast path
+        if (full) {
+            float4 X[V], VX[V];
 #pragma unroll
-        for (int v = 0; v < V; ++v) {
-            const int idx = base + (v * PIC1D_NT + tid) * 4;
-            float4 X = make_float4(0.f, 0.f, 0.f, 0.f), VX = X;
-            if (idx < n_src) {
-                X = __ldcs(reinterpret_cast<const float4*>(a.sx + idx));
-                VX = __ldcs(reinterpret_cast<const float4*>(a.svx + idx));
+            for (int v = 0; v < V; ++v) {
+                const int idx = base + (v * PIC1D_NT + tid) * 4;
+                X[v] = __ldcs(reinterpret_cast<const float4*>(a.sx + idx));
+                VX[v] = __ldcs(reinterpret_cast<const float4*>(a.svx + idx));
             }
-            float xs[4] = {X.x, X.y, X.z, X.w}, vs[4] = {VX.x, VX.y, VX.z, VX.w};
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const int i = idx + c;
-                int key = -3;
-                if (i < n_src) {
-                    key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+            for (int v = 0; v < V; ++v) {
+                float xs[4] = {X[v].x, X[v].y, X[v].z, X[v].w}, vs[4] = {VX[v].x, VX[v].y, VX[v].z, VX[v].w};
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int key = push_particle<BC>(xs[c], vs[c], true, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
                     if (key >= 0) { lo = min(lo, key); hi = max(hi, key); }
                     else if (key == -1) ++ndl;
                     else { ++ndr; nonfinite |= (xs[c] != xs[c]); }
-                    if (a.keys_dbg) a.keys_dbg[i] = key >= 0 ? key : -1;
+                    keys[v * 4 + c] = key;
                 }
-                keys[v * 4 + c] = key;
+            }
+        } else {
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                const int idx = base + (v * PIC1D_NT + tid) * 4;
+                float4 X = make_float4(0.f, 0.f, 0.f, 0.f), VX = X;
+                if (idx < n_src) {
+                    X = __ldcs(reinterpret_cast<const float4*>(a.sx + idx));
+                    VX = __ldcs(reinterpret_cast<const float4*>(a.svx + idx));
+                }
+                float xs[4] = {X.x, X.y, X.z, X.w}, vs[4] = {VX.x, VX.y, VX.z, VX.w};
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int i = idx + c;
+                    int key = -3;
+                    if (i < n_src) {
+                        key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                        if (key >= 0) { lo = min(lo, key); hi = max(hi, key); }
+                        else if (key == -1) ++ndl;
+                        else { ++ndr; nonfinite |= (xs[c] != xs[c]); }
+                        if (a.keys_dbg) a.keys_dbg[i] = key >= 0 ? key : -1;
+                    }
+                    keys[v * 4 + c] = key;
+                }
             }
         }
-        lo = warp_min(lo); hi = warp_max(hi); ndl = warp_sum(ndl); ndr = warp_sum(ndr);
+        lo = __reduce_min_sync(0xffffffffu, lo); hi = __reduce_max_sync(0xffffffffu, hi);
+        ndl = __reduce_add_sync(0xffffffffu, ndl); ndr = __reduce_add_sync(0xffffffffu, ndr);
         if (lane == 0) { s_red[0][wp] = lo; s_red[1][wp] = hi; s_red[2][wp] = ndl; s_red[3][wp] = ndr; }
         if (nonfinite) atomicOr(&a.st->err, ERRBIT_NONFINITE);
         __syncthreads();
         if (tid == 0) {
             int L = 0x7fffffff, H = -1, dl = 0, dr = 0;
+#pragma unroll
             for (int w = 0; w < PIC1D_NWARP; ++w) {
                 L = min(L, s_red[0][w]); H = max(H, s_red[1][w]); dl += s_red[2][w]; dr += s_red[3][w];
             }
@@ -110,68 +137,128 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
         __syncthreads();
         lo = s_bc[0];
         const int w = s_bc[1], off = s_bc[2];
-        // histogram: one shared atomic per run of equal keys; one per warp when the warp is uniform
+        for (int sub = 0; sub < w; sub += WA) {
+            const int nsub = min(WA, w - sub), klo = lo + sub;
+            // histogram: one shared atomic per run of equal keys; one per warp when the warp is uniform
 #pragma unroll
-        for (int v = 0; v < V; ++v) {
-            const int k0 = keys[v * 4], k1 = keys[v * 4 + 1], k2 = keys[v * 4 + 2], k3 = keys[v * 4 + 3];
-            const bool u4 = (k0 >= 0) & (k0 == k1) & (k1 == k2) & (k2 == k3);
-            const int kk = __shfl_sync(0xffffffffu, k0, 0);
-            if (__all_sync(0xffffffffu, u4 && k0 == kk)) {
-                if (lane == 0) atomicAdd(&s_hist[kk], 128);
-            } else {
-                int run = 1;
+            for (int v = 0; v < V; ++v) {
+                const int k0 = keys[v * 4], k1 = keys[v * 4 + 1], k2 = keys[v * 4 + 2], k3 = keys[v * 4 + 3];
+                const bool u4 = (k0 >= 0) & (k0 == k1) & (k1 == k2) & (k2 == k3);
+                const int kk = __shfl_sync(0xffffffffu, k0, 0);
+                if (__all_sync(0xffffffffu, u4 && k0 == kk)) {
+                    if (lane == 0 && (unsigned)(kk - klo) < (unsigned)nsub) atomicAdd(&s_hist[kk - klo], 128);
+                } else {
+                    int run = 1;
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    const int k = keys[v * 4 + c];
-                    const bool last = (c == 3) || (keys[v * 4 + (c < 3 ? c + 1 : 3)] != k);
-                    if (last) { if (k >= 0) atomicAdd(&s_hist[k], run); run = 1; }
-                    else ++run;
+                    for (int c = 0; c < 4; ++c) {
+                        const int k = keys[v * 4 + c];
+                        const bool last = (c == 3) || (keys[v * 4 + (c < 3 ? c + 1 : 3)] != k);
+                        if (last) {
+                            if (k >= 0 && (unsigned)(k - klo) < (unsigned)nsub) atomicAdd(&s_hist[k - klo], run);
+                            run = 1;
+                        } else ++run;
+                    }
                 }
             }
+            __syncthreads();
+            for (int i = tid; i < nsub; i += PIC1D_NT) {
+                if (off >= 0) a.pool[off + sub + i] = s_hist[i];
+                s_hist[i] = 0;
+            }
+            __syncthreads();
         }
-        __syncthreads();
-        for (int i = tid; i < w; i += PIC1D_NT) {
-            if (off >= 0) a.pool[off + i] = s_hist[lo + i];
-            s_hist[lo + i] = 0;
-        }
-        __syncthreads();
     }
 }
 
 // ---- scan over tiles, per sort cell --------------------------------------------------------------
-// thread = one sort cell k.  pool[tile_off[t] + k - tile_lo[t]] becomes the number of particles of
-// tiles < t with key k (exclusive prefix); hist[k] the total.
-__global__ void __launch_bounds__(128) k_bin_scan(SortArgs a) {
-    const int k = blockIdx.x * 128 + threadIdx.x;
-    const int kb0 = blockIdx.x * 128, kb1 = min(kb0 + 127, a.n_sc - 1);
+// Block = 32 adjacent sort cells (lane = cell k) x 32 warps.  The tiles whose window can contain the
+// block's cells form a short range [ta, tb) (found from the tile-group windows); it is split evenly
+// over the warps.  Pass 1 sums each warp's share, a shared-memory prefix orders the warps, pass 2
+// rewrites pool[tile_off[t] + k - tile_lo[t]] as the number of particles of tiles < t with key k
+// (exclusive prefix over tiles); hist[k] gets the total.  Row segments of the pool are read coalesced.
+#define BINSCAN_NW 32
+#define BINSCAN_LIST 4096
+__global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
+    __shared__ int s_wc[BINSCAN_NW];
+    __shared__ unsigned short s_list[BINSCAN_LIST];  // tile groups whose window overlaps the block's cells
+    __shared__ int s_part[BINSCAN_NW][33];
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    const int kb0 = blockIdx.x * 32, kb1 = min(kb0 + 31, a.n_sc - 1);
+    const int k = kb0 + lane;
     const int n_tiles = a.st->sp[a.s].n_tiles;
-    int run = 0;
     const int n_groups = (n_tiles + PIC1D_GROUP - 1) / PIC1D_GROUP;
-    constexpr int B = 8;  // tiles in flight per thread: the loads of a batch are independent
-    for (int g = 0; g < n_groups; ++g) {
-        const int glo = a.grp_lo[g], ghi = a.grp_hi[g];
-        if (ghi < kb0 || glo > kb1) continue;  // block-uniform
-        const int t1 = min((g + 1) * PIC1D_GROUP, n_tiles);
-        for (int t0 = g * PIC1D_GROUP; t0 < t1; t0 += B) {
-            int* p[B];
-            int c[B];
+    // ordered list of the relevant groups (a group is skipped as a whole: the birth tail of a species
+    // has full-width windows and must not drag every tile before it into the walk)
+    int n_rel = 0;
+    for (int g0 = 0; g0 < n_groups; g0 += BINSCAN_NW * 32) {
+        const int g = g0 + tid;
+        const bool rel = g < n_groups && a.grp_hi[g] >= kb0 && a.grp_lo[g] <= kb1;
+        const unsigned bal = __ballot_sync(0xffffffffu, rel);
+        if (lane == 0) s_wc[wp] = __popc(bal);
+        __syncthreads();
+        int before = 0, tot = 0;
+#pragma unroll 8
+        for (int q = 0; q < BINSCAN_NW; ++q) { const int v = s_wc[q]; if (q < wp) before += v; tot += v; }
+        const int idx = n_rel + before + __popc(bal & lanemask_lt());
+        if (rel && idx < BINSCAN_LIST) s_list[idx] = (unsigned short)g;
+        n_rel += tot;
+        __syncthreads();
+    }
+    // n_rel groups (or, if the list overflowed, every group) -> virtual tile range split over the warps
+    const bool listed = n_rel <= BINSCAN_LIST && n_groups <= 65536;
+    const int n_virt = (listed ? n_rel : n_groups) * PIC1D_GROUP;
+    const int chunk = (n_virt + BINSCAN_NW - 1) / BINSCAN_NW;
+    const int v_beg = min(wp * chunk, n_virt), v_end = min(v_beg + chunk, n_virt);
+    constexpr int B = 8;  // tiles in flight per warp: the loads of a batch are independent
+    int sum = 0;
+    for (int v0 = v_beg; v0 < v_end; v0 += B) {
+        int c[B];
 #pragma unroll
-            for (int b = 0; b < B; ++b) {
-                p[b] = nullptr;
-                c[b] = 0;
-                const int t = t0 + b;
-                if (t < t1) {
+        for (int b = 0; b < B; ++b) {
+            c[b] = 0;
+            const int v = v0 + b;
+            if (v < v_end) {
+                const int t = (listed ? (int)s_list[v / PIC1D_GROUP] : v / PIC1D_GROUP) * PIC1D_GROUP + v % PIC1D_GROUP;
+                if (t < n_tiles) {
+                    const unsigned r = (unsigned)(k - a.tile_lo[t]);
+                    if (r < (unsigned)a.tile_w[t]) c[b] = __ldcg(a.pool + a.tile_off[t] + r);
+                }
+            }
+        }
+#pragma unroll
+        for (int b = 0; b < B; ++b) sum += c[b];
+    }
+    s_part[wp][lane] = sum;
+    __syncthreads();
+    int run = 0, total = 0;
+#pragma unroll 8
+    for (int q = 0; q < BINSCAN_NW; ++q) {
+        const int v = s_part[q][lane];
+        if (q < wp) run += v;
+        total += v;
+    }
+    for (int v0 = v_beg; v0 < v_end; v0 += B) {
+        int* p[B];
+        int c[B];
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            p[b] = nullptr;
+            c[b] = 0;
+            const int v = v0 + b;
+            if (v < v_end) {
+                const int t = (listed ? (int)s_list[v / PIC1D_GROUP] : v / PIC1D_GROUP) * PIC1D_GROUP + v % PIC1D_GROUP;
+                if (t < n_tiles) {
                     const unsigned r = (unsigned)(k - a.tile_lo[t]);
                     if (r < (unsigned)a.tile_w[t]) p[b] = a.pool + a.tile_off[t] + r;
                 }
             }
-#pragma unroll
-            for (int b = 0; b < B; ++b) if (p[b]) c[b] = __ldcg(p[b]);
-#pragma unroll
-            for (int b = 0; b < B; ++b) if (p[b]) { __stcg(p[b], run); run += c[b]; }
         }
+#pragma unroll
+        for (int b = 0; b < B; ++b) if (p[b]) c[b] = __ldcg(p[b]);
+#pragma unroll
+        for (int b = 0; b < B; ++b) if (p[b]) { __stcg(p[b], run); run += c[b]; }
     }
-    if (k < a.n_sc) a.hist[k] = run;
+    if (wp == 0 && k < a.n_sc) a.hist[k] = total;
 }
 
 // block-wide exclusive scan of src[0..n) into dst[0..n), returns the total; single block, any n.
@@ -239,9 +326,11 @@ __global__ void __launch_bounds__(1024) k_offsets_scan(SortArgs a) {
 // (measured on sm_100a; a.verify re-checks it with match.any and raises a sticky
 // error).  A per-bin pass then turns the 8 per-warp counts into exclusive prefixes, and
 //     destination = offsets[k] + prefix over earlier tiles [t][k] + prefix over earlier warps + rank.
+// Only x and vx are loaded up front (the push and the key need nothing else); vy and vz are fetched
+// after the ranks are known, so their latency overlaps the per-bin pass and fewer registers are live.
 // Windows wider than WA bins are ranked WA bins at a time.
 template <int BC, int ROWS>
-__global__ void __launch_bounds__(PIC1D_NT) k_push_scatter(SortArgs a) {
+__global__ void __launch_bounds__(PIC1D_NT, (ROWS <= 4 ? 6 : 4)) k_push_scatter(SortArgs a) {
     extern __shared__ unsigned s_mem[];
     const int WA = a.WA;
     unsigned* s_base = s_mem;        // [WA] absolute destination of the tile's first particle per bin
@@ -252,44 +341,50 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_scatter(SortArgs a) {
     unsigned* my_cw = s_cw + (wp >> 1) * WA;
     DevSpecies& sp = a.st->sp[a.s];
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
+    for (int i = tid; i < 4 * WA; i += PIC1D_NT) s_cw[i] = 0u;  // counters are zero between tiles
+    __syncthreads();
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const int lo = a.tile_lo[tile], w = a.tile_w[tile], off = a.tile_off[tile];
         if (off < 0) continue;  // count pool exhausted (sticky ERR_WORKSPACE): drop the tile, write nothing
         const int base = tile * T + wp * (ROWS * 32) + lane;
-        float x[ROWS], vx[ROWS], vy[ROWS], vz[ROWS];
+        const bool full = tile * T + T <= n_push;  // block-uniform
+        float x[ROWS], vx[ROWS];
         int rel[ROWS];  // bin relative to the window; w = absorbed; -1 = no particle / done
         unsigned wall = 0;
+        if (full) {
 #pragma unroll
-        for (int r = 0; r < ROWS; ++r) {
-            const int i = base + r * 32;
-            if (i < n_src) {
-                x[r] = __ldcs(a.sx + i); vx[r] = __ldcs(a.svx + i);
-                vy[r] = __ldcs(a.svy + i); vz[r] = __ldcs(a.svz + i);
+            for (int r = 0; r < ROWS; ++r) { x[r] = __ldcs(a.sx + base + r * 32); vx[r] = __ldcs(a.svx + base + r * 32); }
+        } else {
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) {
+                const int i = base + r * 32;
+                x[r] = 0.0f; vx[r] = 0.0f;
+                if (i < n_src) { x[r] = __ldcs(a.sx + i); vx[r] = __ldcs(a.svx + i); }
             }
         }
+        const int wtot = w + 1;  // + the absorbed "bin"
+        // absolute base of the tile per bin of the first sub-window: in flight together with the particles
+        for (int i = tid; i < min(WA, wtot); i += PIC1D_NT)
+            s_base[i] = i < w ? (unsigned)(a.offsets[lo + i] + __ldcg(a.pool + off + i)) : (unsigned)a.tile_dead[tile];
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
             const int i = base + r * 32;
             rel[r] = -1;
-            if (i < n_src) {
-                const int key = push_particle<BC>(x[r], vx[r], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+            if (full || i < n_src) {
+                const int key = push_particle<BC>(x[r], vx[r], full || i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
                 rel[r] = key >= 0 ? key - lo : w;
                 if (key == -2) wall |= 1u << r;
             }
         }
-        const int wtot = w + 1;  // + the absorbed "bin"
+        float vy[ROWS], vz[ROWS];
         for (int sub = 0; sub < wtot; sub += WA) {
             const int nsub = min(WA, wtot - sub);
-#pragma unroll
-            for (int p = 0; p < 4; ++p)
-                for (int i = tid; i < nsub; i += PIC1D_NT) s_cw[p * WA + i] = 0u;
-            __syncthreads();
             // rank inside the warp's segment
             unsigned ranked = 0;
 #pragma unroll
             for (int r = 0; r < ROWS; ++r) {
                 const int k = rel[r] - sub;
-                const bool in = rel[r] >= 0 && k >= 0 && k < nsub;
+                const bool in = rel[r] >= 0 && k < nsub;  // rel < sub only for particles already scattered (-1)
                 const int k0 = __shfl_sync(0xffffffffu, k, 0);
                 if (__all_sync(0xffffffffu, in && k == k0)) {
                     unsigned old = 0;
@@ -309,12 +404,22 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_scatter(SortArgs a) {
                     ranked |= 1u << r;
                 }
             }
+            if (sub == 0) {  // payload: needed only for the stores
+                if (full) {
+#pragma unroll
+                    for (int r = 0; r < ROWS; ++r) { vy[r] = __ldcs(a.svy + base + r * 32); vz[r] = __ldcs(a.svz + base + r * 32); }
+                } else {
+#pragma unroll
+                    for (int r = 0; r < ROWS; ++r) {
+                        const int i = base + r * 32;
+                        vy[r] = 0.0f; vz[r] = 0.0f;
+                        if (i < n_src) { vy[r] = __ldcs(a.svy + i); vz[r] = __ldcs(a.svz + i); }
+                    }
+                }
+            }
             __syncthreads();
-            // per bin: exclusive prefix over the 8 warps (packed back), absolute base of the tile
+            // per bin: exclusive prefix over the 8 warps (packed back)
             for (int i = tid; i < nsub; i += PIC1D_NT) {
-                const int kk = sub + i;
-                s_base[i] = kk < w ? (unsigned)(a.offsets[lo + kk] + __ldcg(a.pool + off + kk))
-                                   : (unsigned)a.tile_dead[tile];
                 unsigned run = 0;
 #pragma unroll
                 for (int p = 0; p < 4; ++p) {
@@ -339,8 +444,16 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_scatter(SortArgs a) {
                 rel[r] = -1;
             }
             __syncthreads();
+            // zero the counters again; next sub-window's bases
+            for (int i = tid; i < nsub; i += PIC1D_NT) {
+#pragma unroll
+                for (int p = 0; p < 4; ++p) s_cw[p * WA + i] = 0u;
+                const int kk = sub + WA + i;
+                if (kk < wtot)
+                    s_base[i] = kk < w ? (unsigned)(a.offsets[lo + kk] + __ldcg(a.pool + off + kk)) : (unsigned)a.tile_dead[tile];
+            }
+            __syncthreads();
         }
-        __syncthreads();
     }
 }
 
