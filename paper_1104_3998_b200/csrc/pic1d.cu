@@ -227,6 +227,8 @@ int occupancy_grid(pic1d* h, K kernel, size_t smem) {
 }
 
 void setup_launch(pic1d* h) {
+    cudaFuncSetAttribute(k_mcc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
+    cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     h->WA = std::min(h->n_sc + 1, 2048);
     const size_t smem = (size_t)h->WA * sizeof(int);
     h->smem_sort = smem;
@@ -320,7 +322,19 @@ void enqueue_mcc(pic1d* h) {
         m.r_el = (float)c.r_el; m.r_exc = (float)c.r_exc; m.r_ion = (float)c.r_ion;
         m.E_exc = (float)c.E_exc; m.E_ion = (float)c.E_ion;
         m.two_mr = (float)(2.0 * c.mass_ratio); m.gvt = (float)c.gas_vth_ion;
-        k_mcc<<<p.n_mcc_tiles, PIC1D_NT, 0, h->stream>>>(m);
+        // null test in integers: U(w) = (w >> 8) 2^-24 < P0  <=>  (w >> 8) < ceil(P0 2^24)  <=>  w <= null_le
+        const uint64_t thr = (uint64_t)std::ceil((double)m.P0 * 16777216.0) << 8;
+        m.null_any = thr > 0;
+        m.null_le = (uint32_t)(thr - 1);
+        const int grid = std::min(p.n_mcc_tiles, h->num_sms * 4);
+        const bool stage = c.sp[s].P0 > 0.25;
+        if (m.kind == 1) {
+            if (stage) k_mcc<1, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE * sizeof(float), h->stream>>>(m);
+            else k_mcc<1, false><<<grid, PIC1D_NT, MCC_TILE * sizeof(float), h->stream>>>(m);
+        } else {
+            if (stage) k_mcc<2, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE * sizeof(float), h->stream>>>(m);
+            else k_mcc<2, false><<<grid, PIC1D_NT, 0, h->stream>>>(m);
+        }
         mark(h, "mcc", s);
     }
 }

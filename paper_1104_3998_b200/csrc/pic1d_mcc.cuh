@@ -1,16 +1,25 @@
 // pic1d_mcc.cuh -- modified null-collision Monte-Carlo collisions (Eq. 6).
 //
 // Every sorted particle draws p (L203); p < P0 enters the standard null-collision selection with the
-// synthetic analytic cross sections (products and sums only, in the spirit of L207).  One thread
-// handles 4 consecutive sorted slots, so one Philox call serves their 4 null tests (R12).
+// synthetic analytic cross sections (products and sums only, in the spirit of L207).  The paper notes
+// that this module has "lots of branches" (L209); here the branches are removed by compaction inside
+// a tile of MCC_TILE sorted slots:
+//   phase A  null test for every slot: one Philox call serves 4 consecutive slots (R12);
+//            nothing is loaded; candidates are compacted into a shared list
+//   phase B  one thread per CANDIDATE: load v, Philox (u_type, ...), process selection (no
+//            transcendental); real collisions are compacted into a second list
+//   phase C  one thread per REAL COLLISION: kinematics (sqrt, sincos, log), velocity written back
+//   phase D  one thread per IONISATION: the new electron / ion pair
 // Ionisation products go to the tails of the electron / ion arrays in ascending parent-slot order
 // (the paper allocates them with a shared counter inside the parent's sort cell, L203; here the tail
-// is sorted into place by the next step's fine sort).  The cross-block order comes from a decoupled
-// look-back over per-block ionisation counts -- no atomics decide any index.
+// is sorted into place by the next step's fine sort).  The order inside a tile comes from a bit mask
+// over its slots, the order across tiles from a decoupled look-back over per-tile ionisation counts
+// (tiles are handed out by a ticket, so every predecessor of a tile is already running) -- no
+// atomic decides any index.
 #pragma once
 #include "pic1d_device.cuh"
 
-#define MCC_TILE (PIC1D_NT * 4)
+#define MCC_TILE (PIC1D_NT * 16)
 
 struct MccArgs {
     float *x, *vx, *vy, *vz;      // this species' current (sorted) buffer
@@ -21,6 +30,8 @@ struct MccArgs {
     uint8_t* mask;   // optional event mask per sorted slot
     int s, kind, n_species, cap_e, cap_i;
     uint32_t step, k0, k1;
+    uint32_t null_le;  // null test in integers: U(w) < P0  <=>  w <= null_le   (null_any = 0: never)
+    int null_any;
     float P0, inv_g_cap, c_eV, r_el, r_exc, r_ion, E_exc, E_ion, two_mr, gvt;
 };
 
@@ -42,61 +53,105 @@ __device__ __forceinline__ ull desc_pack(uint32_t epoch, ull flag, int v) {
     return ((ull)epoch << 32) | (flag << 30) | (ull)(unsigned)v;
 }
 
-__global__ void __launch_bounds__(PIC1D_NT) k_mcc(MccArgs a) {
+// append `flag`-ged items of a warp to a shared list; returns this lane's index (valid if flag)
+__device__ __forceinline__ int warp_append(bool flag, int* counter) {
+    const unsigned bal = __ballot_sync(0xffffffffu, flag);
+    int base = 0;
+    if ((threadIdx.x & 31) == 0 && bal) base = atomicAdd(counter, __popc(bal));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    return base + __popc(bal & lanemask_lt());
+}
+
+// KIND: 1 electron set, 2 ion charge exchange.  STAGE: phase A streams the tile's vx, vy, vz into shared
+// memory with vector loads while it computes the null tests (worth it when most slots are candidates);
+// otherwise phases B / C fetch the few candidates' velocities from global memory.
+template <int KIND, bool STAGE>
+__global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
+    extern __shared__ float s_v[];  // STAGE: [3][MCC_TILE] velocities; else (KIND 1): [MCC_TILE] speeds of ionising slots
     __shared__ int s_tile, s_excl;
-    __shared__ int s_w[PIC1D_NWARP];
-    __shared__ ull s_cnt[6];
-    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    __shared__ int s_n[3];                          // candidates, real collisions, ionisations
+    __shared__ unsigned short s_cand[MCC_TILE];     // slot - tile base
+    __shared__ unsigned short s_coll[MCC_TILE];     // (slot - tile base) | event << 12
+    __shared__ unsigned s_ionbits[MCC_TILE / 32];   // bit = slot ionises
+    const int tid = threadIdx.x, lane = tid & 31;
     DevState* st = a.st;
     DevSpecies& sp = st->sp[a.s];
-    if (tid == 0) s_tile = atomicAdd(&sp.ticket, 1);
-    if (tid < 6) s_cnt[tid] = 0;
-    __syncthreads();
-    const int tile = s_tile;
     const int n_sorted = sp.n_sorted;
     const int n_act = (n_sorted + MCC_TILE - 1) / MCC_TILE;
-    if (tile >= n_act) return;
-    const int i0 = tile * MCC_TILE + tid * 4;
     const uint32_t epoch = a.step + 1u;
-
-    int ev[4] = {0, 0, 0, 0};
-    float gp_ion[4];
-    int n_cand = 0, n_over = 0, n_ion = 0;
-    if (i0 < n_sorted) {
-        uint32_t w[4];
-        philox4x32_10((uint32_t)(i0 >> 2), a.step, STREAM_NULL + (uint32_t)a.s, 0u, a.k0, a.k1, w);
-        bool cand[4];
-        bool any = false;
+    const uint32_t str_null = STREAM_NULL + (uint32_t)a.s, str_coll = STREAM_COLL + (uint32_t)a.s;
+    int c_cand = 0, c_e0 = 0, c_e1 = 0, c_e2 = 0, c_e3 = 0, c_over = 0;
+    float* s_vx = s_v; float* s_vy = s_v + MCC_TILE; float* s_vz = s_v + 2 * MCC_TILE;
+    unsigned short* s_ion_rel = s_cand;  // ionising slots in slot order (the candidate list is dead by then)
+    float* s_gp = s_v;                   // [slot - tile base] speed shared by the two electrons (its vx is dead by then)
+    while (true) {
+        if (tid == 0) { s_tile = atomicAdd(&sp.ticket, 1); s_n[0] = 0; s_n[1] = 0; s_n[2] = 0; }
+        if (tid < MCC_TILE / 32) s_ionbits[tid] = 0u;
+        __syncthreads();
+        const int tile = s_tile;
+        if (tile >= n_act) break;
+        const int tbase = tile * MCC_TILE;
+        // ---- phase A: null test, 4 slots per Philox call ------------------------------------------
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            cand[c] = (i0 + c < n_sorted) && (u01(w[c]) < a.P0);
-            any |= cand[c];
-        }
-        if (any) {
-            float vx[4], vy[4], vz[4];
-            {
-                const float4 A = *reinterpret_cast<const float4*>(a.vx + i0);
-                const float4 B = *reinterpret_cast<const float4*>(a.vy + i0);
-                const float4 C = *reinterpret_cast<const float4*>(a.vz + i0);
-                vx[0] = A.x; vx[1] = A.y; vx[2] = A.z; vx[3] = A.w;
-                vy[0] = B.x; vy[1] = B.y; vy[2] = B.z; vy[3] = B.w;
-                vz[0] = C.x; vz[1] = C.y; vz[2] = C.z; vz[3] = C.w;
+        for (int q = 0; q < MCC_TILE / (4 * PIC1D_NT); ++q) {
+            const int rel0 = (q * PIC1D_NT + tid) * 4, i0 = tbase + rel0;
+            unsigned bits = 0;
+            if (i0 < n_sorted) {
+                float4 A, B, C;
+                if (STAGE) {  // buffers have capacity slots (a multiple of 4096): the vector never leaves them
+                    A = *reinterpret_cast<const float4*>(a.vx + i0);
+                    B = *reinterpret_cast<const float4*>(a.vy + i0);
+                    C = *reinterpret_cast<const float4*>(a.vz + i0);
+                }
+                uint32_t w[4];
+                philox4x32_10((uint32_t)(i0 >> 2), a.step, str_null, 0u, a.k0, a.k1, w);
+#pragma unroll
+                for (int c = 0; c < 4; ++c)
+                    if (i0 + c < n_sorted && w[c] <= a.null_le) bits |= 1u << c;
+                if (!a.null_any) bits = 0;
+                if (a.mask) *reinterpret_cast<uchar4*>(a.mask + i0) = make_uchar4(0, 0, 0, 0);  // 4-aligned, capacity slots
+                if (STAGE) {
+                    *reinterpret_cast<float4*>(s_vx + rel0) = A;
+                    *reinterpret_cast<float4*>(s_vy + rel0) = B;
+                    *reinterpret_cast<float4*>(s_vz + rel0) = C;
+                }
             }
-            bool changed = false;
+            // ordered append: exclusive prefix of the per-thread counts inside the warp
+            const int cnt = __popc(bits);
+            int inc = cnt;
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                if (!cand[c]) continue;
-                ++n_cand;
-                const uint32_t i = (uint32_t)(i0 + c);
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            int base = 0;
+            if (lane == 31 && inc) base = atomicAdd(&s_n[0], inc);
+            base = __shfl_sync(0xffffffffu, base, 31) + inc - cnt;
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                if ((bits >> c) & 1u) s_cand[base++] = (unsigned short)(rel0 + c);
+        }
+        __syncthreads();
+        // ---- phase B: process selection, one thread per candidate ----------------------------------
+        const int n_cand = s_n[0];
+        c_cand += (tid < n_cand % PIC1D_NT ? 1 : 0) + n_cand / PIC1D_NT;
+        unsigned c_pack = 0;  // four 8-bit event counters of this tile (<= 16 candidates per thread)
+        for (int j0 = 0; j0 < n_cand; j0 += PIC1D_NT) {
+            const int j = j0 + tid;
+            int e = 0;
+            int rel = 0;
+            if (j < n_cand) {
+                rel = s_cand[j];
+                const int i = tbase + rel;
+                const float vx = STAGE ? s_vx[rel] : a.vx[i], vy = STAGE ? s_vy[rel] : a.vy[i], vz = STAGE ? s_vz[rel] : a.vz[i];
                 uint32_t b0[4];
-                philox4x32_10(i, a.step, STREAM_COLL + (uint32_t)a.s, 0u, a.k0, a.k1, b0);
-                const float u_type = u01(b0[0]), u_a = u01(b0[1]), u_b = u01(b0[2]), u_c = u01(b0[3]);
-                const float g2 = __fadd_rn(__fadd_rn(__fmul_rn(vx[c], vx[c]), __fmul_rn(vy[c], vy[c])),
-                                           __fmul_rn(vz[c], vz[c]));
+                philox4x32_10((uint32_t)i, a.step, str_coll, 0u, a.k0, a.k1, b0);
+                const float u_type = u01(b0[0]);
+                const float g2 = __fadd_rn(__fadd_rn(__fmul_rn(vx, vx), __fmul_rn(vy, vy)), __fmul_rn(vz, vz));
                 const float g = sqrtf(g2);
                 const float aa = __fmul_rn(g, a.inv_g_cap);
-                if (aa > 1.0f) ++n_over;
-                if (a.kind == 1) {
+                if (aa > 1.0f) ++c_over;
+                if (KIND == 1) {
                     const float En = __fmul_rn(a.c_eV, g2);
                     const float P_el = __fmul_rn(aa, a.r_el);
                     const float P_exc = En > a.E_exc
@@ -104,165 +159,149 @@ __global__ void __launch_bounds__(PIC1D_NT) k_mcc(MccArgs a) {
                     const float P_ion = En > a.E_ion
                         ? __fmul_rn(__fmul_rn(aa, a.r_ion), __fsub_rn(1.0f, __fdiv_rn(a.E_ion, En))) : 0.0f;
                     const float t1 = P_el, t2 = __fadd_rn(t1, P_exc), t3 = __fadd_rn(t2, P_ion);
-                    const int e = u_type < t1 ? 1 : (u_type < t2 ? 2 : (u_type < t3 ? 3 : 0));
-                    ev[c] = e | 4;  // bit 2: was a candidate
-                    if (e == 0) continue;
-                    float n[3];
-                    iso_dir(u_a, u_b, n);
-                    float gp;
-                    if (e == 1) {
-                        const float dot = __fadd_rn(__fadd_rn(__fmul_rn(n[0], vx[c]), __fmul_rn(n[1], vy[c])),
-                                                    __fmul_rn(n[2], vz[c]));
-                        const float cchi = __fdiv_rn(dot, g);
-                        gp = __fmul_rn(g, sqrtf(__fsub_rn(1.0f, __fmul_rn(a.two_mr, __fsub_rn(1.0f, cchi)))));
-                    } else if (e == 2) {
-                        gp = sqrtf(__fdiv_rn(__fsub_rn(En, a.E_exc), a.c_eV));
-                    } else {
-                        gp = sqrtf(__fdiv_rn(__fmul_rn(__fsub_rn(En, a.E_ion), 0.5f), a.c_eV));
-                        gp_ion[c] = gp;
-                        ++n_ion;
-                    }
-                    vx[c] = __fmul_rn(gp, n[0]); vy[c] = __fmul_rn(gp, n[1]); vz[c] = __fmul_rn(gp, n[2]);
-                    changed = true;
+                    e = u_type < t1 ? 1 : (u_type < t2 ? 2 : (u_type < t3 ? 3 : 0));
                 } else {  // ion charge exchange with the cold background gas
-                    const float P_cx = fminf(1.0f, aa);
-                    const int e = u_type < P_cx ? 1 : 0;
-                    ev[c] = e | 4;
-                    if (e == 0) continue;
-                    uint32_t b1[4];
-                    philox4x32_10(i, a.step, STREAM_COLL + (uint32_t)a.s, 1u, a.k0, a.k1, b1);
-                    const float r12 = bm_r(u_a), ph12 = __fmul_rn(6.2831855f, u_b);
-                    const float r3 = bm_r(u_c), ph3 = __fmul_rn(6.2831855f, u01(b1[0]));
-                    vx[c] = __fmul_rn(a.gvt, __fmul_rn(r12, cosf(ph12)));
-                    vy[c] = __fmul_rn(a.gvt, __fmul_rn(r12, sinf(ph12)));
-                    vz[c] = __fmul_rn(a.gvt, __fmul_rn(r3, cosf(ph3)));
-                    changed = true;
+                    e = u_type < fminf(1.0f, aa) ? 1 : 0;
                 }
+                c_pack += 1u << (8 * e);
+                if (e == 3) atomicOr(&s_ionbits[rel >> 5], 1u << (rel & 31));
+                if (a.mask && e) a.mask[i] = (uint8_t)e;
             }
-            if (changed) {
-                if (i0 + 3 < n_sorted) {
-                    *reinterpret_cast<float4*>(a.vx + i0) = make_float4(vx[0], vx[1], vx[2], vx[3]);
-                    *reinterpret_cast<float4*>(a.vy + i0) = make_float4(vy[0], vy[1], vy[2], vy[3]);
-                    *reinterpret_cast<float4*>(a.vz + i0) = make_float4(vz[0], vz[1], vz[2], vz[3]);
-                } else {  // the group straddles the birth tail: never touch slots >= n_sorted
-#pragma unroll
-                    for (int c = 0; c < 4; ++c)
-                        if (i0 + c < n_sorted) { a.vx[i0 + c] = vx[c]; a.vy[i0 + c] = vy[c]; a.vz[i0 + c] = vz[c]; }
-                }
-            }
+            const int idx = warp_append(e != 0, &s_n[1]);
+            if (e) s_coll[idx] = (unsigned short)(rel | (e << 12));
+            warp_append(e == 3, &s_n[2]);
         }
-        if (a.mask) {
-            uchar4 m = make_uchar4(ev[0] & 3, ev[1] & 3, ev[2] & 3, ev[3] & 3);
-            *reinterpret_cast<uchar4*>(a.mask + i0) = m;  // mask has capacity slots, 4-aligned
-        }
-    }
-    // event counters: warp reduce, then one shared add per warp, one global add per block
-    {
-        int c0 = 0, c1 = 0, c2 = 0, c3 = 0;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            if (ev[c] & 4) { const int e = ev[c] & 3; c0 += e == 0; c1 += e == 1; c2 += e == 2; c3 += e == 3; }
-        }
-        int vals[6] = {n_cand, c0, c1, c2, c3, n_over};
-#pragma unroll
-        for (int q = 0; q < 6; ++q) {
-            const int r = warp_sum(vals[q]);
-            if (lane == 0 && r) atomicAdd(&s_cnt[q], (ull)r);
-        }
-    }
-    // ordered births (electron species only): exclusive prefix of n_ion inside the block ...
-    int inc = n_ion;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) s_w[wp] = inc;
-    __syncthreads();
-    int warp_excl = 0, nb = 0;
-#pragma unroll
-    for (int q = 0; q < PIC1D_NWARP; ++q) { if (q < wp) warp_excl += s_w[q]; nb += s_w[q]; }
-    if (tid == 0) {
-        if (s_cnt[0]) atomicAdd(&sp.n_candidates, s_cnt[0]);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) if (s_cnt[1 + q]) atomicAdd(&sp.n_events[q], s_cnt[1 + q]);
-        if (s_cnt[5]) atomicAdd(&sp.over_cap, s_cnt[5]);
-    }
-    if (a.kind != 1) return;
-    // ... and across blocks by decoupled look-back over the tiles before this one
-    if (tid == 0) {
-        volatile ull* desc = a.desc;
-        int excl = 0;
-        if (tile == 0) {
-            desc[0] = desc_pack(epoch, DESC_PREFIX, nb);
-        } else {
-            desc[tile] = desc_pack(epoch, DESC_AGG, nb);
+        c_e0 += c_pack & 0xff; c_e1 += (c_pack >> 8) & 0xff; c_e2 += (c_pack >> 16) & 0xff; c_e3 += c_pack >> 24;
+        __syncthreads();
+        // ---- publish this tile's ionisation count for the look-back of later tiles ---------------
+        const int nb = s_n[2];
+        if (KIND == 1 && tid == 0) {
+            volatile ull* desc = a.desc;
+            desc[tile] = desc_pack(epoch, tile == 0 ? DESC_PREFIX : DESC_AGG, nb);
             __threadfence();
-            int j = tile - 1;
-            while (true) {
-                const ull d = desc[j];
-                if ((uint32_t)(d >> 32) != epoch) continue;  // not published yet this step
-                const ull flag = (d >> 30) & 3ull;
-                excl += (int)(d & 0x3fffffffull);
-                if (flag == DESC_PREFIX) break;
-                --j;
-            }
-            desc[tile] = desc_pack(epoch, DESC_PREFIX, excl + nb);
         }
-        __threadfence();
-        s_excl = excl;
-        if (tile == n_act - 1) {  // last tile: close the step's birth bookkeeping
-            const int total = excl + nb;
-            const int ne = st->sp[0].n_sorted;
+        // ---- phase C: kinematics, one thread per real collision -------------------------------------
+        const int n_coll = s_n[1];
+        for (int j = tid; j < n_coll; j += PIC1D_NT) {
+            const int rel = s_coll[j] & 0xfff, e = s_coll[j] >> 12;
+            const int i = tbase + rel;
+            uint32_t b0[4];
+            philox4x32_10((uint32_t)i, a.step, str_coll, 0u, a.k0, a.k1, b0);
+            const float u_a = u01(b0[1]), u_b = u01(b0[2]), u_c = u01(b0[3]);
+            if (KIND == 1) {
+                const float vx = STAGE ? s_vx[rel] : a.vx[i], vy = STAGE ? s_vy[rel] : a.vy[i], vz = STAGE ? s_vz[rel] : a.vz[i];
+                const float g2 = __fadd_rn(__fadd_rn(__fmul_rn(vx, vx), __fmul_rn(vy, vy)), __fmul_rn(vz, vz));
+                const float En = __fmul_rn(a.c_eV, g2);
+                float n[3];
+                iso_dir(u_a, u_b, n);
+                float gp;
+                if (e == 1) {
+                    const float g = sqrtf(g2);
+                    const float dot = __fadd_rn(__fadd_rn(__fmul_rn(n[0], vx), __fmul_rn(n[1], vy)), __fmul_rn(n[2], vz));
+                    const float cchi = __fdiv_rn(dot, g);
+                    gp = __fmul_rn(g, sqrtf(__fsub_rn(1.0f, __fmul_rn(a.two_mr, __fsub_rn(1.0f, cchi)))));
+                } else if (e == 2) {
+                    gp = sqrtf(__fdiv_rn(__fsub_rn(En, a.E_exc), a.c_eV));
+                } else {
+                    gp = sqrtf(__fdiv_rn(__fmul_rn(__fsub_rn(En, a.E_ion), 0.5f), a.c_eV));
+                    // rank among the tile's ionisations in slot order
+                    int r = __popc(s_ionbits[rel >> 5] & ((1u << (rel & 31)) - 1u));
+                    for (int q = 0; q < (rel >> 5); ++q) r += __popc(s_ionbits[q]);
+                    s_ion_rel[r] = (unsigned short)rel;
+                    s_gp[rel] = gp;
+                }
+                a.vx[i] = __fmul_rn(gp, n[0]); a.vy[i] = __fmul_rn(gp, n[1]); a.vz[i] = __fmul_rn(gp, n[2]);
+            } else {
+                uint32_t b1[4];
+                philox4x32_10((uint32_t)i, a.step, str_coll, 1u, a.k0, a.k1, b1);
+                const float r12 = bm_r(u_a), ph12 = __fmul_rn(6.2831855f, u_b);
+                const float r3 = bm_r(u_c), ph3 = __fmul_rn(6.2831855f, u01(b1[0]));
+                a.vx[i] = __fmul_rn(a.gvt, __fmul_rn(r12, cosf(ph12)));
+                a.vy[i] = __fmul_rn(a.gvt, __fmul_rn(r12, sinf(ph12)));
+                a.vz[i] = __fmul_rn(a.gvt, __fmul_rn(r3, cosf(ph3)));
+            }
+        }
+        if (KIND != 1) { __syncthreads(); continue; }
+        // ---- ordered births: exclusive prefix over earlier tiles by decoupled look-back --------------
+        if (tid == 0) {
+            volatile ull* desc = a.desc;
+            int excl = 0;
+            if (tile > 0) {
+                int j = tile - 1;
+                while (true) {
+                    const ull d = desc[j];
+                    if ((uint32_t)(d >> 32) != epoch) continue;  // not published yet this step
+                    excl += (int)(d & 0x3fffffffull);
+                    if (((d >> 30) & 3ull) == DESC_PREFIX) break;
+                    --j;
+                }
+                desc[tile] = desc_pack(epoch, DESC_PREFIX, excl + nb);
+                __threadfence();
+            }
+            s_excl = excl;
+            if (tile == n_act - 1) {  // last tile: close the step's birth bookkeeping
+                const int total = excl + nb;
+                const int ne = st->sp[0].n_sorted;
+                int room = a.cap_e - ne;
+                if (a.n_species > 1) room = min(room, a.cap_i - st->sp[1].n_sorted);
+                const int kept = min(total, max(room, 0));
+                st->sp[0].n_live = ne + kept;
+                st->sp[0].births += (ull)kept;
+                if (a.n_species > 1) {
+                    st->sp[1].n_live = st->sp[1].n_sorted + kept;
+                    st->sp[1].births += (ull)kept;
+                }
+                if (total > kept) {
+                    st->sp[0].dropped += (ull)(total - kept);
+                    if (a.n_species > 1) st->sp[1].dropped += (ull)(total - kept);
+                    atomicOr(&st->err, ERRBIT_CAPACITY);
+                }
+            }
+        }
+        __syncthreads();
+        // ---- phase D: one thread per ionisation: the new electron / ion pair -------------------------
+        if (nb > 0) {
+            const int ne = st->sp[0].n_sorted, ni = a.n_species > 1 ? st->sp[1].n_sorted : 0;
             int room = a.cap_e - ne;
-            if (a.n_species > 1) room = min(room, a.cap_i - st->sp[1].n_sorted);
-            const int kept = min(total, max(room, 0));
-            st->sp[0].n_live = ne + kept;
-            st->sp[0].births += (ull)kept;
-            if (a.n_species > 1) {
-                st->sp[1].n_live = st->sp[1].n_sorted + kept;
-                st->sp[1].births += (ull)kept;
-            }
-            if (total > kept) {
-                st->sp[0].dropped += (ull)(total - kept);
-                if (a.n_species > 1) st->sp[1].dropped += (ull)(total - kept);
-                atomicOr(&st->err, ERRBIT_CAPACITY);
+            if (a.n_species > 1) room = min(room, a.cap_i - ni);
+            for (int r = tid; r < nb; r += PIC1D_NT) {
+                const int b = s_excl + r;  // birth index of the step, ascending parent slot
+                if (b >= room) continue;
+                const uint32_t i = (uint32_t)(tbase + s_ion_rel[r]);
+                uint32_t b0[4], b1[4], b2[4];
+                philox4x32_10(i, a.step, str_coll, 0u, a.k0, a.k1, b0);
+                philox4x32_10(i, a.step, str_coll, 1u, a.k0, a.k1, b1);
+                philox4x32_10(i, a.step, str_coll, 2u, a.k0, a.k1, b2);
+                const float xp = a.x[i];
+                float n2[3];
+                iso_dir(u01(b0[3]), u01(b1[0]), n2);
+                const float gp = s_gp[s_ion_rel[r]];
+                const int de = ne + b;
+                a.ex[de] = xp;
+                a.evx[de] = __fmul_rn(gp, n2[0]); a.evy[de] = __fmul_rn(gp, n2[1]); a.evz[de] = __fmul_rn(gp, n2[2]);
+                if (a.n_species > 1) {
+                    const float r12 = bm_r(u01(b1[1])), ph12 = __fmul_rn(6.2831855f, u01(b1[2]));
+                    const float r3 = bm_r(u01(b1[3])), ph3 = __fmul_rn(6.2831855f, u01(b2[0]));
+                    const int di = ni + b;
+                    a.ix[di] = xp;
+                    a.ivx[di] = __fmul_rn(a.gvt, __fmul_rn(r12, cosf(ph12)));
+                    a.ivy[di] = __fmul_rn(a.gvt, __fmul_rn(r12, sinf(ph12)));
+                    a.ivz[di] = __fmul_rn(a.gvt, __fmul_rn(r3, cosf(ph3)));
+                }
             }
         }
+        __syncthreads();
     }
-    if (nb == 0) return;  // block-uniform
-    __syncthreads();
-    if (n_ion == 0) return;
-    int b = s_excl + warp_excl + inc - n_ion;  // birth index of this thread's first ionisation
-    const int ne = st->sp[0].n_sorted, ni = a.n_species > 1 ? st->sp[1].n_sorted : 0;
-    int room = a.cap_e - ne;
-    if (a.n_species > 1) room = min(room, a.cap_i - ni);
+    // event counters: warp reduce, one global add per warp
+    {
+        int vals[6] = {c_cand, c_e0, c_e1, c_e2, c_e3, c_over};
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        if ((ev[c] & 3) != 3) continue;
-        if (b < room) {
-            const uint32_t i = (uint32_t)(i0 + c);
-            uint32_t b0[4], b1[4], b2[4];
-            philox4x32_10(i, a.step, STREAM_COLL + (uint32_t)a.s, 0u, a.k0, a.k1, b0);
-            philox4x32_10(i, a.step, STREAM_COLL + (uint32_t)a.s, 1u, a.k0, a.k1, b1);
-            philox4x32_10(i, a.step, STREAM_COLL + (uint32_t)a.s, 2u, a.k0, a.k1, b2);
-            const float xp = a.x[i];
-            float n2[3];
-            iso_dir(u01(b0[3]), u01(b1[0]), n2);
-            const float gp = gp_ion[c];
-            const int de = ne + b;
-            a.ex[de] = xp;
-            a.evx[de] = __fmul_rn(gp, n2[0]); a.evy[de] = __fmul_rn(gp, n2[1]); a.evz[de] = __fmul_rn(gp, n2[2]);
-            if (a.n_species > 1) {
-                const float r12 = bm_r(u01(b1[1])), ph12 = __fmul_rn(6.2831855f, u01(b1[2]));
-                const float r3 = bm_r(u01(b1[3])), ph3 = __fmul_rn(6.2831855f, u01(b2[0]));
-                const int di = ni + b;
-                a.ix[di] = xp;
-                a.ivx[di] = __fmul_rn(a.gvt, __fmul_rn(r12, cosf(ph12)));
-                a.ivy[di] = __fmul_rn(a.gvt, __fmul_rn(r12, sinf(ph12)));
-                a.ivz[di] = __fmul_rn(a.gvt, __fmul_rn(r3, cosf(ph3)));
-            }
+        for (int q = 0; q < 6; ++q) vals[q] = __reduce_add_sync(0xffffffffu, vals[q]);
+        if (lane == 0) {
+            if (vals[0]) atomicAdd(&sp.n_candidates, (ull)vals[0]);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) if (vals[1 + q]) atomicAdd(&sp.n_events[q], (ull)vals[1 + q]);
+            if (vals[5]) atomicAdd(&sp.over_cap, (ull)vals[5]);
         }
-        ++b;
     }
 }
