@@ -59,8 +59,10 @@ struct pic1d {
     bool ready;
     int64_t launches;
     cudaError_t last_err;
-    int grid_count, grid_scatter, WA;
-    size_t smem_sort, smem_scatter;
+    int grid_count, grid_scatter[2], WA;
+    size_t smem_sort, smem_scatter[2];
+    void (*k_count)(SortArgs);
+    void (*k_scatter[2])(SortArgs);
     bool timing;
     std::vector<TimeMark> marks;
     std::vector<cudaEvent_t> ev_pool;
@@ -207,19 +209,26 @@ SortArgs sort_args(pic1d* h, int s) {
     return a;
 }
 
-template <int BC>
-void launch_count(pic1d* h, const SortArgs& a, int grid) {
-    if (h->T == 2048) k_push_count<BC, 2><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a);
-    else k_push_count<BC, 1><<<grid, PIC1D_NT, h->smem_sort, h->stream>>>(a);
-}
-template <int BC>
-void launch_scatter(pic1d* h, const SortArgs& a, int grid) {
-    if (h->T == 2048) k_push_scatter<BC, 8><<<grid, PIC1D_NT, h->smem_scatter, h->stream>>>(a);
-    else k_push_scatter<BC, 4><<<grid, PIC1D_NT, h->smem_scatter, h->stream>>>(a);
+typedef void (*sort_kernel_t)(SortArgs);
+
+sort_kernel_t count_kernel(int bc, int T) {
+    if (bc == 1) return T == 2048 ? k_push_count<1, 2> : k_push_count<1, 1>;
+    return T == 2048 ? k_push_count<0, 2> : k_push_count<0, 1>;
 }
 
-template <class K>
-int occupancy_grid(pic1d* h, K kernel, size_t smem) {
+// abs: the species records its absorbed slots (ions with secondary emission); stage: the species may
+// spread a tile over many bins (electrons), see k_push_scatter
+sort_kernel_t scatter_kernel(int bc, int T, bool abs, bool stage) {
+    if (bc == 1) {
+        if (stage) return T == 2048 ? k_push_scatter<1, 8, false, true> : k_push_scatter<1, 4, false, true>;
+        return T == 2048 ? k_push_scatter<1, 8, false, false> : k_push_scatter<1, 4, false, false>;
+    }
+    if (abs) return T == 2048 ? k_push_scatter<0, 8, true, false> : k_push_scatter<0, 4, true, false>;
+    if (stage) return T == 2048 ? k_push_scatter<0, 8, false, true> : k_push_scatter<0, 4, false, true>;
+    return T == 2048 ? k_push_scatter<0, 8, false, false> : k_push_scatter<0, 4, false, false>;
+}
+
+int occupancy_grid(pic1d* h, sort_kernel_t kernel, size_t smem) {
     if (smem > 48 * 1024) cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     int nb = 1;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, PIC1D_NT, smem);
@@ -229,21 +238,17 @@ int occupancy_grid(pic1d* h, K kernel, size_t smem) {
 void setup_launch(pic1d* h) {
     cudaFuncSetAttribute(k_mcc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
-    h->WA = std::min(h->n_sc + 1, 2048);
-    const size_t smem = (size_t)h->WA * sizeof(int);
-    h->smem_sort = smem;
-    const size_t sm2 = (size_t)h->WA * 5 * sizeof(unsigned);
-    h->smem_scatter = sm2;
-    int gc, gs;
-    if (h->cfg.bc == 1) {
-        if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<1, 2>, smem); gs = occupancy_grid(h, k_push_scatter<1, 8>, sm2); }
-        else { gc = occupancy_grid(h, k_push_count<1, 1>, smem); gs = occupancy_grid(h, k_push_scatter<1, 4>, sm2); }
-    } else {
-        if (h->T == 2048) { gc = occupancy_grid(h, k_push_count<0, 2>, smem); gs = occupancy_grid(h, k_push_scatter<0, 8>, sm2); }
-        else { gc = occupancy_grid(h, k_push_count<0, 1>, smem); gs = occupancy_grid(h, k_push_scatter<0, 4>, sm2); }
+    h->WA = std::min((h->n_sc + 1 + 3) / 4 * 4, 1024);
+    h->smem_sort = (size_t)h->WA * sizeof(int);
+    h->k_count = count_kernel(h->cfg.bc, h->T);
+    h->grid_count = occupancy_grid(h, h->k_count, h->smem_sort);
+    for (int s = 0; s < h->cfg.n_species; ++s) {
+        const bool abs = s == 1 && h->abs_list != nullptr;
+        const bool stage = s == 0;
+        h->k_scatter[s] = scatter_kernel(h->cfg.bc, h->T, abs, stage);
+        h->smem_scatter[s] = (size_t)h->WA * 9 * sizeof(unsigned) + (stage ? (size_t)h->T * 18 : 0);
+        h->grid_scatter[s] = occupancy_grid(h, h->k_scatter[s], h->smem_scatter[s]);
     }
-    h->grid_count = gc;
-    h->grid_scatter = gs;
 }
 
 // fine sort of species s (mode 0: no push)
@@ -254,14 +259,14 @@ void enqueue_sort(pic1d* h, int s, int shift = 0) {
         a.shift = shift;
         a.n_sc = ((h->n_sc - 1) >> shift) + 1;
     }
-    const int gc = std::min(h->grid_count, p.n_tiles_max), gs = std::min(h->grid_scatter, p.n_tiles_max);
-    if (h->cfg.bc == 1) launch_count<1>(h, a, gc); else launch_count<0>(h, a, gc);
+    const int gc = std::min(h->grid_count, p.n_tiles_max), gs = std::min(h->grid_scatter[s], p.n_tiles_max);
+    h->k_count<<<gc, PIC1D_NT, h->smem_sort, h->stream>>>(a);
     mark(h, "push_count", s);
     k_bin_scan<<<(a.n_sc + 31) / 32, BINSCAN_NW * 32, 0, h->stream>>>(a);
     mark(h, "bin_scan", s);
     k_offsets_scan<<<1, 1024, 0, h->stream>>>(a);
     mark(h, "offsets_scan", s);
-    if (h->cfg.bc == 1) launch_scatter<1>(h, a, gs); else launch_scatter<0>(h, a, gs);
+    h->k_scatter[s]<<<gs, PIC1D_NT, h->smem_scatter[s], h->stream>>>(a);
     mark(h, "push_scatter", s);
     p.cur ^= 1;
 }

@@ -35,6 +35,8 @@ struct DevSpecies {
     int n_dead;    // absorbed particles of the running sort
     int pool_used; // entries of the (tile x bin) count pool in use
     int ticket;    // dynamic tile counter of the MCC kernel
+    int ticket2;   // dynamic tile counter of the scatter kernel
+    int pad_;
     ull absorbed_left, absorbed_right, injected, n_candidates, n_events[4], births, dropped, over_cap;
 };
 

@@ -317,39 +317,54 @@ __global__ void __launch_bounds__(1024) k_offsets_scan(SortArgs a) {
 }
 
 // ---- pass 2 -----------------------------------------------------------------------------------
-// ROWS rows of 32 consecutive slots per warp: tile T = NT * ROWS.
+// ROWS rows of 32 consecutive slots per warp: tile T = NT * ROWS.  Tiles are handed out by a ticket,
+// so the blocks advance through the source as one narrow front and the destination lines they share
+// meet in L2.
 //
 // Stable rank inside the tile without any serial section: every warp owns ROWS*32 consecutive slots
-// and a private counter per bin of the tile's window (two warps share a 32-bit word, 16 bits each).
-// A shared-memory atomicAdd returns the rank inside the warp's segment: rows are issued in slot
-// order, and lanes of one instruction that hit the same counter are served in ascending lane order
-// (measured on sm_100a; a.verify re-checks it with match.any and raises a sticky
-// error).  A per-bin pass then turns the 8 per-warp counts into exclusive prefixes, and
+// and a private 32-bit counter per bin of the tile's window.  A shared-memory atomicAdd returns the
+// rank inside the warp's segment: rows are issued in slot order, and lanes of one instruction that
+// hit the same counter are served in ascending lane order (measured on sm_100a, DESIGN.md "Kernels";
+// a.verify re-checks it with match.any and raises a sticky error).  A per-bin pass (4 bins per
+// thread, 128-bit shared accesses) then turns the 8 per-warp counts into per-warp bases, and
 //     destination = offsets[k] + prefix over earlier tiles [t][k] + prefix over earlier warps + rank.
 // Only x and vx are loaded up front (the push and the key need nothing else); vy and vz are fetched
 // after the ranks are known, so their latency overlaps the per-bin pass and fewer registers are live.
-// Windows wider than WA bins are ranked WA bins at a time.
-template <int BC, int ROWS>
-__global__ void __launch_bounds__(PIC1D_NT, (ROWS <= 4 ? 6 : 4)) k_push_scatter(SortArgs a) {
+//
+// STAGE (electrons): when the tile's particles spread over many bins (runs shorter than 64 slots:
+// particles move many cells per step, Eq. 5 violated), the per-bin pass also scans the bin totals,
+// the particles are first placed in tile-sorted order in shared memory and then copied out by
+// consecutive threads, so that a warp's store covers a few runs instead of 32 separate sectors.
+// ABS (ions with secondary emission): absorbed particles form a pseudo-bin after the window and are
+// written, in slot order, to the absorbed list.  Windows wider than WA bins are ranked WA bins at a
+// time (direct scatter).
+template <int BC, int ROWS, bool ABS, bool STAGE>
+__global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k_push_scatter(SortArgs a) {
     extern __shared__ unsigned s_mem[];
-    const int WA = a.WA;
+    __shared__ int s_tile;
+    __shared__ unsigned s_scan[PIC1D_NWARP + 1];
+    const int WA = a.WA;             // a multiple of 4
     unsigned* s_base = s_mem;        // [WA] absolute destination of the tile's first particle per bin
-    unsigned* s_cw = s_mem + WA;     // [4][WA] per warp-pair packed counters, then exclusive prefixes
+    unsigned* s_cnt = s_mem + WA;    // [8][WA] per-warp counters, then per-warp bases
     constexpr int T = PIC1D_NT * ROWS;
+    float* s_st = reinterpret_cast<float*>(s_mem + 9 * WA);                   // STAGE: [4][T]
+    unsigned short* s_key = reinterpret_cast<unsigned short*>(s_st + 4 * T);  // STAGE: [T]
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
-    const int sh = (wp & 1) * 16;
-    unsigned* my_cw = s_cw + (wp >> 1) * WA;
+    unsigned* my = s_cnt + wp * WA;
     DevSpecies& sp = a.st->sp[a.s];
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
-    for (int i = tid; i < 4 * WA; i += PIC1D_NT) s_cw[i] = 0u;  // counters are zero between tiles
+    for (int i = tid; i < 8 * WA; i += PIC1D_NT) s_cnt[i] = 0u;  // counters are zero between tiles
+    if (tid == 0) s_tile = atomicAdd(&sp.ticket2, 1);
     __syncthreads();
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    while (true) {
+        const int tile = s_tile;
+        if (tile >= n_tiles) break;
         const int lo = a.tile_lo[tile], w = a.tile_w[tile], off = a.tile_off[tile];
-        if (off < 0) continue;  // count pool exhausted (sticky ERR_WORKSPACE): drop the tile, write nothing
         const int base = tile * T + wp * (ROWS * 32) + lane;
         const bool full = tile * T + T <= n_push;  // block-uniform
-        float x[ROWS], vx[ROWS];
-        int rel[ROWS];  // bin relative to the window; w = absorbed; -1 = no particle / done
+        const int wtot = off < 0 ? 0 : (ABS ? w + 1 : w);  // off < 0: count pool exhausted (sticky error), drop the tile
+        float x[ROWS], vx[ROWS], vy[ROWS], vz[ROWS];
+        int rel[ROWS];  // bin relative to the window; w = absorbed (ABS); -1 = no particle / done
         unsigned wall = 0;
         if (full) {
 #pragma unroll
@@ -362,7 +377,6 @@ __global__ void __launch_bounds__(PIC1D_NT, (ROWS <= 4 ? 6 : 4)) k_push_scatter(
                 if (i < n_src) { x[r] = __ldcs(a.sx + i); vx[r] = __ldcs(a.svx + i); }
             }
         }
-        const int wtot = w + 1;  // + the absorbed "bin"
         // absolute base of the tile per bin of the first sub-window: in flight together with the particles
         for (int i = tid; i < min(WA, wtot); i += PIC1D_NT)
             s_base[i] = i < w ? (unsigned)(a.offsets[lo + i] + __ldcg(a.pool + off + i)) : (unsigned)a.tile_dead[tile];
@@ -372,14 +386,14 @@ __global__ void __launch_bounds__(PIC1D_NT, (ROWS <= 4 ? 6 : 4)) k_push_scatter(
             rel[r] = -1;
             if (full || i < n_src) {
                 const int key = push_particle<BC>(x[r], vx[r], full || i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
-                rel[r] = key >= 0 ? key - lo : w;
-                if (key == -2) wall |= 1u << r;
+                rel[r] = key >= 0 ? key - lo : (ABS ? w : -1);
+                if (ABS && key == -2) wall |= 1u << r;
             }
         }
-        float vy[ROWS], vz[ROWS];
+        const bool staged = STAGE && !ABS && wtot <= WA && wtot >= T / 64;  // block-uniform
         for (int sub = 0; sub < wtot; sub += WA) {
             const int nsub = min(WA, wtot - sub);
-            // rank inside the warp's segment
+            // ---- rank inside the warp's segment ---------------------------------------------------
             unsigned ranked = 0;
 #pragma unroll
             for (int r = 0; r < ROWS; ++r) {
@@ -388,13 +402,12 @@ __global__ void __launch_bounds__(PIC1D_NT, (ROWS <= 4 ? 6 : 4)) k_push_scatter(
                 const int k0 = __shfl_sync(0xffffffffu, k, 0);
                 if (__all_sync(0xffffffffu, in && k == k0)) {
                     unsigned old = 0;
-                    if (lane == 0) old = atomicAdd(&my_cw[k0], 32u << sh);
+                    if (lane == 0) old = atomicAdd(&my[k0], 32u);
                     old = __shfl_sync(0xffffffffu, old, 0);
-                    rel[r] = k | ((int)(((old >> sh) & 0xffffu) + lane) << 16);
+                    rel[r] = k | ((int)(old + lane) << 16);
                     ranked |= 1u << r;
                 } else if (in) {
-                    const unsigned old = atomicAdd(&my_cw[k], 1u << sh);
-                    const int rank = (int)((old >> sh) & 0xffffu);
+                    const int rank = (int)atomicAdd(&my[k], 1u);
                     if (a.verify) {
                         const unsigned peers = __match_any_sync(__activemask(), k);
                         const int first = __shfl_sync(peers, rank, __ffs(peers) - 1);
@@ -418,42 +431,103 @@ __global__ void __launch_bounds__(PIC1D_NT, (ROWS <= 4 ? 6 : 4)) k_push_scatter(
                 }
             }
             __syncthreads();
-            // per bin: exclusive prefix over the 8 warps (packed back)
-            for (int i = tid; i < nsub; i += PIC1D_NT) {
-                unsigned run = 0;
+            // ---- per bin: counts of the 8 warps -> bases of the 8 warps ------------------------------
+            // direct: base = absolute destination; staged: base = position in the tile-sorted order,
+            // and s_base becomes (absolute destination - position of the bin's first particle)
+            unsigned n_out = 0;
+            {
+                const int i4 = tid * 4;
+                const bool act = i4 < nsub;
+                uint4 tot = make_uint4(0u, 0u, 0u, 0u);
+                if (act) {
 #pragma unroll
-                for (int p = 0; p < 4; ++p) {
-                    const unsigned word = s_cw[p * WA + i];
-                    const unsigned c0 = word & 0xffffu, c1 = word >> 16;
-                    s_cw[p * WA + i] = run | ((run + c0) << 16);
-                    run += c0 + c1;
+                    for (int q = 0; q < PIC1D_NWARP; ++q) {
+                        const uint4 c = *reinterpret_cast<const uint4*>(s_cnt + q * WA + i4);
+                        tot.x += c.x; tot.y += c.y; tot.z += c.z; tot.w += c.w;
+                    }
+                }
+                uint4 b4 = make_uint4(0u, 0u, 0u, 0u);
+                if (act) b4 = *reinterpret_cast<const uint4*>(s_base + i4);
+                if (staged) {  // block-wide exclusive scan of the bin totals
+                    const unsigned S = tot.x + tot.y + tot.z + tot.w;
+                    unsigned inc = S;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
+                        if (lane >= o) inc += t;
+                    }
+                    if (lane == 31) s_scan[wp] = inc;
+                    __syncthreads();
+                    unsigned before = 0, all = 0;
+#pragma unroll
+                    for (int q = 0; q < PIC1D_NWARP; ++q) { const unsigned v = s_scan[q]; if (q < wp) before += v; all += v; }
+                    n_out = all;
+                    const unsigned e0 = before + inc - S;
+                    const uint4 ls = make_uint4(e0, e0 + tot.x, e0 + tot.x + tot.y, e0 + tot.x + tot.y + tot.z);
+                    if (act)
+                        *reinterpret_cast<uint4*>(s_base + i4) = make_uint4(b4.x - ls.x, b4.y - ls.y, b4.z - ls.z, b4.w - ls.w);
+                    b4 = ls;
+                }
+                if (act) {
+#pragma unroll
+                    for (int q = 0; q < PIC1D_NWARP; ++q) {  // counts are re-read: keeping them would spill
+                        const uint4 c = *reinterpret_cast<const uint4*>(s_cnt + q * WA + i4);
+                        *reinterpret_cast<uint4*>(s_cnt + q * WA + i4) = b4;
+                        b4.x += c.x; b4.y += c.y; b4.z += c.z; b4.w += c.w;
+                    }
                 }
             }
             __syncthreads();
-            // scatter: destination = tile base of the bin + prefix over earlier warps + rank in the warp
+            if (!staged) {
+                // ---- direct scatter: destination = base of (warp, bin) + rank in the warp ------------
 #pragma unroll
-            for (int r = 0; r < ROWS; ++r) {
-                if (!((ranked >> r) & 1u)) continue;
-                const int k = rel[r] & 0xffff, rank = rel[r] >> 16;
-                const unsigned d = s_base[k] + ((my_cw[k] >> sh) & 0xffffu) + (unsigned)rank;
-                if (sub + k < w) {
-                    a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
-                } else if (a.abs_list && (int)d < a.abs_cap) {  // absorbed: ordered list of (slot, wall)
-                    a.abs_list[d] = (unsigned)(base + r * 32) | (((wall >> r) & 1u) << 31);
+                for (int r = 0; r < ROWS; ++r) {
+                    if (!((ranked >> r) & 1u)) continue;
+                    const int k = rel[r] & 0xffff;
+                    const unsigned d = my[k] + (unsigned)(rel[r] >> 16);
+                    if (!ABS || sub + k < w) {
+                        a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
+                    } else if (a.abs_list && (int)d < a.abs_cap) {  // absorbed: ordered list of (slot, wall)
+                        a.abs_list[d] = (unsigned)(base + r * 32) | (((wall >> r) & 1u) << 31);
+                    }
+                    rel[r] = -1;
                 }
-                rel[r] = -1;
-            }
-            __syncthreads();
-            // zero the counters again; next sub-window's bases
-            for (int i = tid; i < nsub; i += PIC1D_NT) {
+            } else {
+                // ---- staged: tile-sorted order in shared memory, then coalesced copy-out ----------------
 #pragma unroll
-                for (int p = 0; p < 4; ++p) s_cw[p * WA + i] = 0u;
-                const int kk = sub + WA + i;
-                if (kk < wtot)
-                    s_base[i] = kk < w ? (unsigned)(a.offsets[lo + kk] + __ldcg(a.pool + off + kk)) : (unsigned)a.tile_dead[tile];
+                for (int r = 0; r < ROWS; ++r) {
+                    if (!((ranked >> r) & 1u)) continue;
+                    const int k = rel[r] & 0xffff;
+                    const unsigned li = my[k] + (unsigned)(rel[r] >> 16);
+                    s_st[li] = x[r]; s_st[T + li] = vx[r]; s_st[2 * T + li] = vy[r]; s_st[3 * T + li] = vz[r];
+                    s_key[li] = (unsigned short)k;
+                    rel[r] = -1;
+                }
+                __syncthreads();
+                for (int j = tid; j < (int)n_out; j += PIC1D_NT) {
+                    const unsigned d = s_base[s_key[j]] + (unsigned)j;
+                    a.dx[d] = s_st[j]; a.dvx[d] = s_st[T + j]; a.dvy[d] = s_st[2 * T + j]; a.dvz[d] = s_st[3 * T + j];
+                }
             }
             __syncthreads();
+            // ---- zero the counters again; next sub-window's bases ---------------------------------------
+            {
+                const int i4 = tid * 4;
+                if (i4 < nsub) {
+#pragma unroll
+                    for (int q = 0; q < PIC1D_NWARP; ++q)
+                        *reinterpret_cast<uint4*>(s_cnt + q * WA + i4) = make_uint4(0u, 0u, 0u, 0u);
+                }
+                for (int i = tid; i < nsub; i += PIC1D_NT) {
+                    const int kk = sub + WA + i;
+                    if (kk < wtot)
+                        s_base[i] = kk < w ? (unsigned)(a.offsets[lo + kk] + __ldcg(a.pool + off + kk)) : (unsigned)a.tile_dead[tile];
+                }
+            }
+            if (sub + WA < wtot) __syncthreads();
         }
+        if (tid == 0) s_tile = atomicAdd(&sp.ticket2, 1);
+        __syncthreads();
     }
 }
 
@@ -471,6 +545,7 @@ __global__ void k_step_begin(DevState* st, int n_species, int mode, int T, int* 
             sp.n_dead = 0;
             sp.pool_used = 0;
             sp.ticket = 0;
+            sp.ticket2 = 0;
         }
         st->n_abs = 0;
     }
