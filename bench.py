@@ -172,6 +172,7 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_1104_3998_b200 import pic1d as G
+    from paper_1104_3998_b200 import replicas as R
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -182,7 +183,7 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     # replicas only: rank r runs its own discharge (seed + r) on its own GPU
-    p["seed"] = p["seed"] + rank
+    p["seed"] = R.replica_seed(p["seed"], rank)
     parts = W.make_particles(p)
     pinned = [[torch.from_numpy(a).pin_memory() for a in sp] for sp in parts]
     sim = G.Pic1D(p, device=dev)
@@ -216,13 +217,8 @@ def main():
     launches = sim.launch_count - l0
     m1 = live()
     n_mean = 0.5 * (sum(m["count"] for m in m0) + sum(m["count"] for m in m1))
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    tot = torch.tensor([n_mean], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    ms_max, n_total = float(t.item()), float(tot.item())
-    value = n_total * args.steps / (ms_max * 1e-3)
+    ms_max, n_total = R.reduce_replicas(ms, n_mean, dev)
+    value = R.throughput(n_total, args.steps, ms_max)
 
     if args.profile:
         if rank == 0:
@@ -303,10 +299,8 @@ def main():
         e2e_step()
     barrier()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = n_e2e * world * args.e2e_steps / float(te.item())
+    e2e_ms, n_e2e_total = R.reduce_replicas(e2e_s * 1e3, n_e2e, dev)
+    e2e_value = R.throughput(n_e2e_total, args.e2e_steps, e2e_ms)
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
