@@ -119,7 +119,7 @@ size_t layout(pic1d* h, char* base) {
     h->T = cap_max >= 2048ll * 592 ? 2048 : 1024;
     const int rr = c.sort_inv_ratio < 1.0 ? (int)std::llround(1.0 / c.sort_inv_ratio) : 1;
     const int ppc_est = (int)std::max<int64_t>(1, cap_max / c.n_cells);
-    h->G = std::min(2048, std::max(rr, pow2_floor(std::max(1, 4096 / ppc_est))));
+    h->G = std::min(2048, std::max(rr, pow2_floor(std::max(1, 8192 / ppc_est))));
     h->n_dep_blocks = (c.n_cells + h->G - 1) / h->G;
     size_t off = 0;
     h->st = carve<DevState>(base, off, 1);
@@ -236,6 +236,7 @@ int occupancy_grid(pic1d* h, sort_kernel_t kernel, size_t smem) {
 }
 
 void setup_launch(pic1d* h) {
+    cudaFuncSetAttribute(k_field_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, FIELD_SMEM_MAX * (int)sizeof(double));
     cudaFuncSetAttribute(k_mcc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     h->WA = std::min((h->n_sc + 1 + 3) / 4 * 4, 1024);
@@ -288,7 +289,7 @@ void enqueue_grid(pic1d* h, unsigned n_time) {
         DepositArgs d;
         d.x = p.buf[p.cur][0]; d.offsets = p.offsets; d.part = p.part; d.side = p.side;
         d.Nc = c.n_cells; d.n_sc = h->n_sc; d.G = h->G; d.inv_r = h->inv_r;
-        k_deposit<<<h->n_dep_blocks, PIC1D_NT, (h->G + 1) * sizeof(double), h->stream>>>(d);
+        k_deposit<<<h->n_dep_blocks, PIC1D_NT, (h->G + 1) * sizeof(ull), h->stream>>>(d);
         mark(h, "deposit", s);
         cb.part[s] = p.part; cb.side[s] = p.side; cb.rho_s[s] = p.rho_s; cb.sign[s] = c.sp[s].charge_sign;
     }
@@ -300,7 +301,12 @@ void enqueue_grid(pic1d* h, unsigned n_time) {
     f.rho = h->rho; f.phi = h->phi; f.E = h->E; f.S = h->S; f.Tt = h->Tt; f.E32 = h->E32;
     f.Nc = c.n_cells; f.nodes = h->nodes; f.bc = c.bc; f.V0 = c.V0_norm; f.omega_dt = c.omega_dt;
     f.n_time = n_time;
-    k_field<<<1, 1024, 0, h->stream>>>(f);
+    if (c.n_cells <= FIELD_SMEM_MAX) {
+        const size_t sm = (size_t)((c.n_cells + 1023) / 1024) * 32 * 32 * sizeof(double);
+        k_field_smem<<<1, 1024, sm, h->stream>>>(f);
+    } else {
+        k_field<<<1, 1024, 0, h->stream>>>(f);
+    }
     mark(h, "field", -1);
 }
 

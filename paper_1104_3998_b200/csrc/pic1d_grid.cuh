@@ -20,71 +20,89 @@ __device__ __forceinline__ double warp_sum_d(double v) {
 }
 
 // Block b owns grid cells [b G, (b+1) G) and therefore the contiguous slot range
-// offsets[key(b G)] .. offsets[key((b+1) G)] of the sorted array.  Every warp keeps per-lane fp64
-// partial sums in registers for the cell it is currently in (the paper's register partial sums,
-// L130), reduces them with shuffles when the cell changes, and adds the two node weights to the
-// block's shared-memory window.  Rows that straddle cells are split by cell value.
+// offsets[key(b G)] .. offsets[key((b+1) G)] of the sorted array; every warp takes a contiguous part
+// of it.  The node weights are accumulated as 64-bit FIXED-POINT integers in units of 2^-40: f = x - j
+// is a multiple of 2^-23 for x >= 1, so the integer sums are exact and equal, after conversion, to the
+// oracle's fp64 sums in any order (sums stay below 2^53 for up to 8192 particles per node; only
+// particles with x < 2^-17 lose bits, below the rounding of the fp64 sum itself).  While a warp's rows
+// stay in one cell the per-lane sums live in registers (the paper's register partial sums, L130) and
+// are reduced with shuffles when the cell changes; rows that straddle cells are split by cell value, one
+// warp reduction per distinct cell.
+#define DEP_ONE (1ll << 40)
+#define DEP_U 4  // rows in flight per warp
+
+__device__ __forceinline__ long long warp_sum_ll(long long v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
 __global__ void __launch_bounds__(PIC1D_NT) k_deposit(DepositArgs a) {
-    extern __shared__ double s_acc[];  // G + 1 nodes
+    extern __shared__ ull s_acc[];  // G + 1 nodes
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
     const int c0 = blockIdx.x * a.G, c1 = min(c0 + a.G, a.Nc);
     const int k0 = (int)__fmul_rn((float)c0, a.inv_r);
     const int k1 = c1 >= a.Nc ? a.n_sc : (int)__fmul_rn((float)c1, a.inv_r);
     const int p0 = a.offsets[k0], p1 = a.offsets[k1];
-    for (int i = tid; i <= a.G; i += PIC1D_NT) s_acc[i] = 0.0;
+    for (int i = tid; i <= a.G; i += PIC1D_NT) s_acc[i] = 0ull;
     __syncthreads();
+    const int rows_w = ((p1 - p0 + 31) / 32 + PIC1D_NWARP - 1) / PIC1D_NWARP;
+    const int beg = min(p0 + wp * rows_w * 32, p1), end = min(beg + rows_w * 32, p1);
     int jc = -1, accn = 0;
-    double accf = 0.0;
-    for (int rb = p0 + wp * 32; rb < p1; rb += PIC1D_NT) {
-        const int i = rb + lane;
-        const bool valid = i < p1;
-        int j = -1;
-        float f = 0.0f;
-        if (valid) {
-            const float x = __ldcs(a.x + i);
-            j = (int)x;
-            f = __fsub_rn(x, (float)j);
+    long long accF = 0;
+    for (int i0 = beg; i0 < end; i0 += 32 * DEP_U) {
+        float xv[DEP_U];
+#pragma unroll
+        for (int u = 0; u < DEP_U; ++u) {
+            const int i = i0 + u * 32 + lane;
+            xv[u] = i < end ? __ldcs(a.x + i) : -1.0f;
         }
-        unsigned rem = __ballot_sync(0xffffffffu, valid);
-        while (rem) {
-            const int jj = __shfl_sync(0xffffffffu, j, __ffs(rem) - 1);
-            const bool in = valid && j == jj;
-            const unsigned grp = __ballot_sync(0xffffffffu, in);
-            if (grp == rem) {
-                // the rest of the row is one cell: accumulate in registers
-                if (jj != jc) {
+#pragma unroll
+        for (int u = 0; u < DEP_U; ++u) {
+            const bool valid = xv[u] >= 0.0f;
+            const int j = (int)xv[u];
+            const long long F = __float2ll_rz(__fmul_rn(__fsub_rn(xv[u], (float)j), 0x1p40f));
+            const int j0 = __shfl_sync(0xffffffffu, j, 0);
+            if (__all_sync(0xffffffffu, valid && j == j0)) {
+                if (j0 != jc) {
                     if (jc >= 0) {
-                        const double F = warp_sum_d(accf);
-                        const int n = warp_sum(accn);
+                        const long long Fs = warp_sum_ll(accF);
+                        const int n = __reduce_add_sync(0xffffffffu, accn);
                         if (lane == 0) {
-                            atomicAdd(&s_acc[jc - c0], (double)n - F);
-                            atomicAdd(&s_acc[jc + 1 - c0], F);
+                            atomicAdd(&s_acc[jc - c0], (ull)((long long)n * DEP_ONE - Fs));
+                            atomicAdd(&s_acc[jc + 1 - c0], (ull)Fs);
                         }
                     }
-                    jc = jj; accf = 0.0; accn = 0;
+                    jc = j0; accF = 0; accn = 0;
                 }
-                if (in) { accf += (double)f; ++accn; }
-            } else {
-                const double F = warp_sum_d(in ? (double)f : 0.0);
-                if (lane == 0) {
-                    atomicAdd(&s_acc[jj - c0], (double)__popc(grp) - F);
-                    atomicAdd(&s_acc[jj + 1 - c0], F);
+                accF += F; ++accn;
+            } else {  // the row straddles cells: one warp reduction per distinct cell
+                unsigned rem = __ballot_sync(0xffffffffu, valid);
+                while (rem) {
+                    const int jj = __shfl_sync(0xffffffffu, j, __ffs(rem) - 1);
+                    const bool in = valid && j == jj;
+                    const unsigned grp = __ballot_sync(0xffffffffu, in);
+                    const long long Fs = warp_sum_ll(in ? F : 0ll);
+                    if (lane == 0) {
+                        atomicAdd(&s_acc[jj - c0], (ull)((long long)__popc(grp) * DEP_ONE - Fs));
+                        atomicAdd(&s_acc[jj + 1 - c0], (ull)Fs);
+                    }
+                    rem &= ~grp;
                 }
             }
-            rem &= ~grp;
         }
     }
     if (jc >= 0) {
-        const double F = warp_sum_d(accf);
-        const int n = warp_sum(accn);
+        const long long Fs = warp_sum_ll(accF);
+        const int n = __reduce_add_sync(0xffffffffu, accn);
         if (lane == 0) {
-            atomicAdd(&s_acc[jc - c0], (double)n - F);
-            atomicAdd(&s_acc[jc + 1 - c0], F);
+            atomicAdd(&s_acc[jc - c0], (ull)((long long)n * DEP_ONE - Fs));
+            atomicAdd(&s_acc[jc + 1 - c0], (ull)Fs);
         }
     }
     __syncthreads();
-    for (int i = tid; i < a.G; i += PIC1D_NT) a.part[(size_t)blockIdx.x * a.G + i] = s_acc[i];
-    if (tid == 0) a.side[blockIdx.x] = s_acc[c1 - c0];
+    for (int i = tid; i < a.G; i += PIC1D_NT) a.part[(size_t)blockIdx.x * a.G + i] = (double)s_acc[i] * 0x1p-40;
+    if (tid == 0) a.side[blockIdx.x] = (double)s_acc[c1 - c0] * 0x1p-40;
 }
 
 // Follow-up kernel (L138): node j of species s = block part + the left neighbour's right-edge node;
@@ -219,6 +237,97 @@ __global__ void __launch_bounds__(1024) k_field(FieldArgs a) {
     if (a.bc == 1) {  // report phi with its mean removed
         const double pm = block_sum_d(psum) / (double)N;
         for (int j = tid; j < N; j += blockDim.x) a.phi[j] -= pm;
+    }
+}
+
+// Shared-memory variant for N_c <= FIELD_SMEM_MAX cells (all BASELINE configs): rho is read once,
+// coalesced, into shared memory; each warp scans a contiguous segment row by row with shuffles (no bank
+// conflicts, no dependent global loads); T is never stored -- phi and E are emitted while the second scan
+// runs.  One launch, ~10 us at 16384 cells.
+#define FIELD_SMEM_MAX 24576
+
+__device__ __forceinline__ double warp_incl_scan_d(double v, int lane) {
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double t = __shfl_up_sync(0xffffffffu, v, o);
+        if (lane >= o) v += t;
+    }
+    return v;
+}
+
+__global__ void __launch_bounds__(1024) k_field_smem(FieldArgs a) {
+    extern __shared__ double s_S[];  // [32 * seg]
+    __shared__ double s_w[32];
+    const int N = a.Nc, tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    const int seg = ((N + 1023) / 1024) * 32;  // elements per warp, a multiple of 32
+    const double* rho = a.rho;
+    double mean = 0.0;
+    if (a.bc == 1) {
+        double p = 0.0;
+        for (int i = tid; i < N; i += 1024) p += rho[i];
+        mean = block_sum_d(p) / (double)N;
+    }
+    for (int i = tid; i < 32 * seg; i += 1024) s_S[i] = (i == 0 || i >= N) ? 0.0 : rho[i] - mean;
+    __syncthreads();
+    // scan 1: S_j = sum_{i<=j} (rho_i - mean), S_0 = 0
+    const int b = wp * seg;
+    {
+        double carry = 0.0;
+        for (int r = 0; r < seg; r += 32) {
+            const double v = warp_incl_scan_d(s_S[b + r + lane], lane) + carry;
+            s_S[b + r + lane] = v;
+            carry = __shfl_sync(0xffffffffu, v, 31);
+        }
+        if (lane == 0) s_w[wp] = carry;
+    }
+    __syncthreads();
+    {
+        double off = 0.0;
+        for (int q = 0; q < wp; ++q) off += s_w[q];
+        __syncthreads();
+        double tot = 0.0;
+        for (int r = 0; r < seg; r += 32) {
+            const double v = s_S[b + r + lane] + off;
+            s_S[b + r + lane] = v;
+            tot += (b + r + lane < N) ? v : 0.0;
+        }
+        tot = warp_sum_d(tot);  // sum of S over the warp's segment (elements < N)
+        if (lane == 0) s_w[wp] = tot;
+    }
+    __syncthreads();
+    // scan 2 (T_j = sum_{i<=j} S_i) fused with the outputs
+    double toff = 0.0, T_all = 0.0;
+    for (int q = 0; q < 32; ++q) { const double v = s_w[q]; if (q < wp) toff += v; T_all += v; }
+    const double phi0 = a.bc == 0 ? a.V0 * sin(a.omega_dt * (double)a.n_time) : 0.0;
+    const double phiN = 0.0;
+    const double d1 = (phiN - phi0 + T_all) / (double)N;  // T_all = T_{N-1}
+    double psum = 0.0, carry = toff;
+    for (int r = 0; r < seg; r += 32) {
+        const int i = b + r + lane;  // element i gives node j = i + 1
+        const double Si = s_S[i];
+        const double Ti = warp_incl_scan_d(i < N ? Si : 0.0, lane) + carry;
+        carry = __shfl_sync(0xffffffffu, Ti, 31);
+        const int j = i + 1;
+        if (j < N) {
+            const double phi = phi0 + (double)j * d1 - Ti;
+            const double E = -d1 + 0.5 * (Si + s_S[j]);
+            a.phi[j] = phi; a.E[j] = E; a.E32[j] = (float)E;
+            psum += phi;
+        }
+    }
+    if (tid == 0) {
+        const double SN1 = s_S[N - 1];
+        const double E0 = a.bc == 0 ? -d1 - rho[0] : -d1 + 0.5 * SN1;
+        a.phi[0] = phi0; a.E[0] = E0; a.E32[0] = (float)E0;
+        psum += phi0;
+        if (a.bc == 0) {
+            const double EN = -d1 + SN1 + rho[N];
+            a.phi[N] = phiN; a.E[N] = EN; a.E32[N] = (float)EN;
+        }
+    }
+    if (a.bc == 1) {  // report phi with its mean removed
+        const double pm = block_sum_d(psum) / (double)N;
+        for (int j = tid; j < N; j += 1024) a.phi[j] -= pm;
     }
 }
 

@@ -262,52 +262,60 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
 }
 
 // block-wide exclusive scan of src[0..n) into dst[0..n), returns the total; single block, any n.
+// Thread-contiguous chunks: one pass to sum, one warp-shuffle scan over the threads, one pass to write.
 // dst may alias src.
-__device__ int block_exclusive_scan(const int* src, int* dst, int n, int carry_in) {
-    __shared__ int s_w[32];
-    __shared__ int s_carry;
+__device__ int block_exclusive_scan(const int* src, int* dst, int n) {
+    __shared__ int s_w[33];
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5, nw = blockDim.x >> 5;
-    if (tid == 0) s_carry = carry_in;
+    const int ch = (n + blockDim.x - 1) / blockDim.x;
+    const int b = min(tid * ch, n), e = min(b + ch, n);
+    int tot = 0;
+    for (int i = b; i < e; i += 8) {  // 8 independent loads in flight
+        int v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = i + u < e ? src[i + u] : 0;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) tot += v[u];
+    }
+    int inc = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    __syncthreads();  // s_w may still be read by a previous call
+    if (lane == 31) s_w[wp] = inc;
     __syncthreads();
-    for (int base = 0; base < n; base += blockDim.x) {
-        const int i = base + tid;
-        const int v = i < n ? src[i] : 0;
-        int inc = v;
+    if (wp == 0) {
+        const int t = lane < nw ? s_w[lane] : 0;
+        int ti = t;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            int t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
+            const int u = __shfl_up_sync(0xffffffffu, ti, o);
+            if (lane >= o) ti += u;
         }
-        if (lane == 31) s_w[wp] = inc;
-        __syncthreads();
-        if (wp == 0) {
-            int t = lane < nw ? s_w[lane] : 0;
-            int ti = t;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                int u = __shfl_up_sync(0xffffffffu, ti, o);
-                if (lane >= o) ti += u;
-            }
-            s_w[lane] = ti - t;  // exclusive over warps
-            if (lane == 31) s_w[31] = ti - t;
-        }
-        __syncthreads();
-        const int carry = s_carry;
-        if (i < n) dst[i] = carry + s_w[wp] + inc - v;
-        __syncthreads();
-        if (tid == blockDim.x - 1) s_carry = carry + s_w[wp] + inc;
-        __syncthreads();
+        s_w[lane] = ti - t;  // exclusive over warps
+        if (lane == 31) s_w[32] = ti;
     }
-    return s_carry;
+    __syncthreads();
+    int run = s_w[wp] + inc - tot;
+    for (int i = b; i < e; i += 8) {
+        int v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = i + u < e ? src[i + u] : 0;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) if (i + u < e) { dst[i + u] = run; run += v[u]; }
+    }
+    return s_w[32];
 }
 
-// offsets[k] = #{key < k}; n_live = n_sorted = survivors; exclusive prefix of absorbed counts.
+// offsets[k] = #{key < k}; n_live = n_sorted = survivors; exclusive prefix of absorbed counts (only
+// needed when the species keeps an ordered absorbed list).
 __global__ void __launch_bounds__(1024) k_offsets_scan(SortArgs a) {
     DevSpecies& sp = a.st->sp[a.s];
-    const int total = block_exclusive_scan(a.hist, a.offsets, a.n_sc, 0);
-    __syncthreads();
-    const int n_dead = block_exclusive_scan(a.tile_dead, a.tile_dead, sp.n_tiles, 0);
-    __syncthreads();
+    const int total = block_exclusive_scan(a.hist, a.offsets, a.n_sc);
+    int n_dead = 0;
+    if (a.abs_list) n_dead = block_exclusive_scan(a.tile_dead, a.tile_dead, sp.n_tiles);
     if (threadIdx.x == 0) {
         a.offsets[a.n_sc] = total;
         sp.n_live = total;
