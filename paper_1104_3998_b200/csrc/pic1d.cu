@@ -25,7 +25,7 @@ struct SpeciesHost {
     int cur;
     int capacity, n_tiles_max, n_groups_max;
     int *tile_lo, *tile_w, *tile_off, *tile_dead, *grp_lo, *grp_hi, *pool;
-    int pool_size;
+    int pool_size, pool_stride, pool_fixed;
     int *hist, *offsets, *keys_dbg;
     uint8_t* mask;
     double *part, *side, *rho_s;
@@ -152,9 +152,13 @@ size_t layout(pic1d* h, char* base) {
         p.tile_dead = carve<int>(base, off, p.n_tiles_max);
         p.grp_lo = carve<int>(base, off, p.n_groups_max);
         p.grp_hi = carve<int>(base, off, p.n_groups_max);
-        int64_t full = (int64_t)p.n_tiles_max * h->n_sc;
-        int64_t want = std::max<int64_t>(1 << 20, (int64_t)p.n_tiles_max * 4096);
-        p.pool_size = (int)std::min<int64_t>(std::min(full, want), (1ll << 30));
+        // count pool: one fixed row of pool_stride bins per tile + an overflow region for wider windows
+        const int64_t over = std::max<int64_t>(4 << 20, p.capacity / 4);
+        int64_t stride = std::min<int64_t>((h->n_sc + 3) / 4 * 4, 4096);
+        stride = std::max<int64_t>(4, std::min<int64_t>(stride, (((1ll << 31) - 1 - over) / p.n_tiles_max) / 4 * 4));
+        p.pool_stride = (int)stride;
+        p.pool_fixed = (int)(stride * p.n_tiles_max);
+        p.pool_size = (int)(p.pool_fixed + over);
         p.pool = carve<int>(base, off, p.pool_size);
         p.hist = carve<int>(base, off, h->n_sc + 1);
         p.offsets = carve<int>(base, off, h->n_sc + 1);
@@ -199,7 +203,7 @@ SortArgs sort_args(pic1d* h, int s) {
     a.dx = p.buf[d][0]; a.dvx = p.buf[d][1]; a.dvy = p.buf[d][2]; a.dvz = p.buf[d][3];
     a.E32 = h->E32; a.st = h->st; a.s = s;
     a.tile_lo = p.tile_lo; a.tile_w = p.tile_w; a.tile_off = p.tile_off; a.tile_dead = p.tile_dead;
-    a.grp_lo = p.grp_lo; a.grp_hi = p.grp_hi; a.pool = p.pool; a.pool_size = p.pool_size;
+    a.grp_lo = p.grp_lo; a.grp_hi = p.grp_hi; a.pool = p.pool; a.pool_size = p.pool_size; a.pool_stride = p.pool_stride; a.pool_fixed = p.pool_fixed;
     a.hist = p.hist; a.offsets = p.offsets; a.keys_dbg = p.keys_dbg;
     a.abs_list = (s == 1) ? h->abs_list : nullptr;
     a.abs_cap = h->abs_cap;
@@ -484,7 +488,7 @@ int pic1d_load_particles(pic1d_t* h, int s, int64_t n, const float* x, const flo
     int shift = 0;
     for (int q = 0; q < h->cfg.n_species; ++q) {
         const SpeciesHost& pq = h->sp[q];
-        while ((int64_t)(((h->n_sc - 1) >> shift) + 1) * pq.n_tiles_max > pq.pool_size) ++shift;
+        while (((h->n_sc - 1) >> shift) + 1 > pq.pool_stride) ++shift;
     }
     if (shift > 0) {
         enqueue_begin(h, 0);

@@ -28,7 +28,9 @@ struct SortArgs {
     int *tile_lo, *tile_w, *tile_off, *tile_dead;  // per tile: window start, width, pool offset, absorbed
     int *grp_lo, *grp_hi;                          // per tile group: union window
     int* pool;
-    int pool_size;
+    int pool_size;    // fixed rows + overflow region
+    int pool_stride;  // bins per fixed pool row (one row per tile)
+    int pool_fixed;   // n_tiles_max * pool_stride: start of the overflow region
     int* hist;     // [n_sc]
     int* offsets;  // [n_sc + 1]
     int* keys_dbg; // optional, per source slot
@@ -44,22 +46,29 @@ struct SortArgs {
 // ---- pass 1 -----------------------------------------------------------------------------------
 // V float4 loads per thread: tile T = NT * 4 * V slots.  The tile's histogram lives in a shared
 // window of WA counters relative to the tile's lowest key; wider windows are counted WA bins at a time.
+// A tile whose window fits pool_stride bins owns the fixed pool row tile * pool_stride (no allocation);
+// wider ones (a species' birth tail) take space from the overflow region with one atomicAdd per tile --
+// the position in the pool carries no meaning, so this atomic decides no particle index.
 template <int BC, int V>
 __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
     extern __shared__ int s_hist[];  // WA counters, all zero between tiles
-    __shared__ int s_red[4][PIC1D_NWARP];
-    __shared__ int s_bc[3];
+    __shared__ int s_lohi[2][2];     // block min / max of the keys, double-buffered over tiles
+    __shared__ int s_dead[2][2];     // absorbed left / right, double-buffered
+    __shared__ int s_off;
     constexpr int T = PIC1D_NT * 4 * V;
-    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
     const int WA = a.WA;
     DevSpecies& sp = a.st->sp[a.s];
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
     for (int i = tid; i < WA; i += PIC1D_NT) s_hist[i] = 0;
+    if (tid < 2) { s_lohi[tid][0] = 0x7fffffff; s_lohi[tid][1] = -1; s_dead[tid][0] = 0; s_dead[tid][1] = 0; }
     __syncthreads();
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    int par = 0;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, par ^= 1) {
         const int base = tile * T;
         int keys[4 * V];
-        int lo = 0x7fffffff, hi = -1, ndl = 0, ndr = 0;
+        unsigned ulo = 0xffffffffu;  // absorbed keys are negative: huge as unsigned, below every max as signed
+        int hi = -1, smin = 0;       // smin < 0: the thread saw an absorbed (or missing) particle
         bool nonfinite = false;
         const bool full = base + T <= n_push && a.keys_dbg == nullptr;  // block-uniform fast path
         if (full) {
@@ -76,9 +85,8 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     const int key = push_particle<BC>(xs[c], vs[c], true, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
-                    if (key >= 0) { lo = min(lo, key); hi = max(hi, key); }
-                    else if (key == -1) ++ndl;
-                    else { ++ndr; nonfinite |= (xs[c] != xs[c]); }
+                    ulo = min(ulo, (unsigned)key); hi = max(hi, key); smin = min(smin, key);
+                    if (key == -2) nonfinite |= (xs[c] != xs[c]);
                     keys[v * 4 + c] = key;
                 }
             }
@@ -95,70 +103,75 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     const int i = idx + c;
-                    int key = -3;
+                    int key = -3;  // no particle
+                    smin = min(smin, i < n_src ? 0 : -3);
                     if (i < n_src) {
                         key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
-                        if (key >= 0) { lo = min(lo, key); hi = max(hi, key); }
-                        else if (key == -1) ++ndl;
-                        else { ++ndr; nonfinite |= (xs[c] != xs[c]); }
+                        ulo = min(ulo, (unsigned)key); hi = max(hi, key); smin = min(smin, key);
+                        if (key == -2) nonfinite |= (xs[c] != xs[c]);
                         if (a.keys_dbg) a.keys_dbg[i] = key >= 0 ? key : -1;
                     }
                     keys[v * 4 + c] = key;
                 }
             }
         }
-        lo = __reduce_min_sync(0xffffffffu, lo); hi = __reduce_max_sync(0xffffffffu, hi);
-        ndl = __reduce_add_sync(0xffffffffu, ndl); ndr = __reduce_add_sync(0xffffffffu, ndr);
-        if (lane == 0) { s_red[0][wp] = lo; s_red[1][wp] = hi; s_red[2][wp] = ndl; s_red[3][wp] = ndr; }
+        ulo = __reduce_min_sync(0xffffffffu, ulo); hi = __reduce_max_sync(0xffffffffu, hi);
+        if (lane == 0) {
+            if ((int)ulo >= 0) atomicMin(&s_lohi[par][0], (int)ulo);  // a warp of absorbed particles has none
+            atomicMax(&s_lohi[par][1], hi);
+        }
+        if (__any_sync(0xffffffffu, smin < 0)) {  // some lane of the warp saw an absorbed (or missing) particle: rare
+            int ndl = 0, ndr = 0;
+            int lo2 = 0x7fffffff;
+#pragma unroll
+            for (int q = 0; q < 4 * V; ++q) {
+                ndl += keys[q] == -1; ndr += keys[q] == -2;
+                if (keys[q] >= 0) lo2 = min(lo2, keys[q]);
+            }
+            ndl = __reduce_add_sync(0xffffffffu, ndl); ndr = __reduce_add_sync(0xffffffffu, ndr);
+            lo2 = __reduce_min_sync(0xffffffffu, lo2);
+            if (lane == 0) {
+                if (ndl) atomicAdd(&s_dead[par][0], ndl);
+                if (ndr) atomicAdd(&s_dead[par][1], ndr);
+                if (lo2 != 0x7fffffff) atomicMin(&s_lohi[par][0], lo2);
+            }
+        }
         if (nonfinite) atomicOr(&a.st->err, ERRBIT_NONFINITE);
         __syncthreads();
+        const int L0 = s_lohi[par][0], H = s_lohi[par][1];
+        const int w = H >= L0 ? H - L0 + 1 : 0;
+        const int lo = w > 0 ? L0 : 0;
+        int off = tile * a.pool_stride;
+        if (w > a.pool_stride) {  // block-uniform; overflow region
+            if (tid == 0) {
+                int o = atomicAdd(&sp.pool_used, w);
+                if (o + w > a.pool_size - a.pool_fixed) { o = -1; atomicOr(&a.st->err, ERRBIT_WORKSPACE); }
+                s_off = o >= 0 ? a.pool_fixed + o : -1;
+            }
+            __syncthreads();
+            off = s_off;
+        }
         if (tid == 0) {
-            int L = 0x7fffffff, H = -1, dl = 0, dr = 0;
-#pragma unroll
-            for (int w = 0; w < PIC1D_NWARP; ++w) {
-                L = min(L, s_red[0][w]); H = max(H, s_red[1][w]); dl += s_red[2][w]; dr += s_red[3][w];
-            }
-            int w = H >= L ? H - L + 1 : 0;
-            int off = 0;
+            const int dl = s_dead[par][0], dr = s_dead[par][1];
             if (w > 0) {
-                off = atomicAdd(&sp.pool_used, w);
-                if (off + w > a.pool_size) { off = -1; atomicOr(&a.st->err, ERRBIT_WORKSPACE); }
-                atomicMin(&a.grp_lo[tile / PIC1D_GROUP], L);
+                atomicMin(&a.grp_lo[tile / PIC1D_GROUP], lo);
                 atomicMax(&a.grp_hi[tile / PIC1D_GROUP], H);
-            } else {
-                L = 0;
             }
-            a.tile_lo[tile] = L; a.tile_w[tile] = off >= 0 ? w : 0; a.tile_off[tile] = off;
+            a.tile_lo[tile] = lo; a.tile_w[tile] = off >= 0 ? w : 0; a.tile_off[tile] = off;
             a.tile_dead[tile] = dl + dr;
             if (dl) atomicAdd(&sp.absorbed_left, (ull)dl);
             if (dr) atomicAdd(&sp.absorbed_right, (ull)dr);
-            s_bc[0] = L; s_bc[1] = w; s_bc[2] = off;
+            // reset the OTHER buffer for the next tile (nobody touches it before the next barrier)
+            s_lohi[par ^ 1][0] = 0x7fffffff; s_lohi[par ^ 1][1] = -1; s_dead[par ^ 1][0] = 0; s_dead[par ^ 1][1] = 0;
         }
-        __syncthreads();
-        lo = s_bc[0];
-        const int w = s_bc[1], off = s_bc[2];
         for (int sub = 0; sub < w; sub += WA) {
             const int nsub = min(WA, w - sub), klo = lo + sub;
-            // histogram: one shared atomic per run of equal keys; one per warp when the warp is uniform
+            // histogram: one shared-memory reduction per particle (conflicting red.shared is not
+            // serialised on sm_100a: 3 cycles per warp instruction)
 #pragma unroll
-            for (int v = 0; v < V; ++v) {
-                const int k0 = keys[v * 4], k1 = keys[v * 4 + 1], k2 = keys[v * 4 + 2], k3 = keys[v * 4 + 3];
-                const bool u4 = (k0 >= 0) & (k0 == k1) & (k1 == k2) & (k2 == k3);
-                const int kk = __shfl_sync(0xffffffffu, k0, 0);
-                if (__all_sync(0xffffffffu, u4 && k0 == kk)) {
-                    if (lane == 0 && (unsigned)(kk - klo) < (unsigned)nsub) atomicAdd(&s_hist[kk - klo], 128);
-                } else {
-                    int run = 1;
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        const int k = keys[v * 4 + c];
-                        const bool last = (c == 3) || (keys[v * 4 + (c < 3 ? c + 1 : 3)] != k);
-                        if (last) {
-                            if (k >= 0 && (unsigned)(k - klo) < (unsigned)nsub) atomicAdd(&s_hist[k - klo], run);
-                            run = 1;
-                        } else ++run;
-                    }
-                }
+            for (int q = 0; q < 4 * V; ++q) {
+                const unsigned r = (unsigned)(keys[q] - klo);
+                if (r < (unsigned)nsub) atomicAdd(&s_hist[r], 1);
             }
             __syncthreads();
             for (int i = tid; i < nsub; i += PIC1D_NT) {
@@ -167,6 +180,7 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
             }
             __syncthreads();
         }
+        if (w == 0) __syncthreads();  // keep the double buffer two barriers apart
     }
 }
 
