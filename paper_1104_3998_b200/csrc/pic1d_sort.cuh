@@ -276,29 +276,25 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
 }
 
 // block-wide exclusive scan of src[0..n) into dst[0..n), returns the total; single block, any n.
-// Thread-contiguous chunks: one pass to sum, one warp-shuffle scan over the threads, one pass to write.
+// Every warp owns a contiguous segment and walks it in rows of 32 (coalesced): pass 1 sums the
+// segment (independent loads), a shuffle scan orders the warps, pass 2 scans row by row with a carry.
 // dst may alias src.
 __device__ int block_exclusive_scan(const int* src, int* dst, int n) {
     __shared__ int s_w[33];
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5, nw = blockDim.x >> 5;
-    const int ch = (n + blockDim.x - 1) / blockDim.x;
-    const int b = min(tid * ch, n), e = min(b + ch, n);
+    const int seg = ((n + nw * 32 - 1) / (nw * 32)) * 32;  // elements per warp, a multiple of 32
+    const int b = min(wp * seg, n), e = min(b + seg, n);
     int tot = 0;
-    for (int i = b; i < e; i += 8) {  // 8 independent loads in flight
+    for (int i = b + lane; i < e; i += 32 * 8) {
         int v[8];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) v[u] = i + u < e ? src[i + u] : 0;
+        for (int u = 0; u < 8; ++u) v[u] = i + u * 32 < e ? src[i + u * 32] : 0;
 #pragma unroll
         for (int u = 0; u < 8; ++u) tot += v[u];
     }
-    int inc = tot;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += t;
-    }
+    tot = __reduce_add_sync(0xffffffffu, tot);
     __syncthreads();  // s_w may still be read by a previous call
-    if (lane == 31) s_w[wp] = inc;
+    if (lane == 0) s_w[wp] = tot;
     __syncthreads();
     if (wp == 0) {
         const int t = lane < nw ? s_w[lane] : 0;
@@ -312,13 +308,22 @@ __device__ int block_exclusive_scan(const int* src, int* dst, int n) {
         if (lane == 31) s_w[32] = ti;
     }
     __syncthreads();
-    int run = s_w[wp] + inc - tot;
-    for (int i = b; i < e; i += 8) {
-        int v[8];
+    int carry = s_w[wp];
+    for (int i0 = b; i0 < e; i0 += 32 * 4) {
+        int v[4];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) v[u] = i + u < e ? src[i + u] : 0;
+        for (int u = 0; u < 4; ++u) v[u] = i0 + u * 32 + lane < e ? src[i0 + u * 32 + lane] : 0;
 #pragma unroll
-        for (int u = 0; u < 8; ++u) if (i + u < e) { dst[i + u] = run; run += v[u]; }
+        for (int u = 0; u < 4; ++u) {
+            int inc = v[u];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            if (i0 + u * 32 + lane < e) dst[i0 + u * 32 + lane] = carry + inc - v[u];
+            carry += __shfl_sync(0xffffffffu, inc, 31);
+        }
     }
     return s_w[32];
 }
