@@ -163,7 +163,8 @@ enum pic1d_debug_what {
     PIC1D_DBG_OFFSETS = 5, /* int32[N_sc + 1] */
     PIC1D_DBG_MASK = 6,    /* uint8 per sorted slot: MCC event of the last step (needs CAPTURE) */
     PIC1D_DBG_E32 = 7,     /* float[n_nodes]: the field the next push will gather */
-    PIC1D_DBG_RHO_S = 8    /* double[n_nodes]: rho_s of the last deposit */
+    PIC1D_DBG_RHO_S = 8,   /* double[n_nodes]: rho_s of the last deposit */
+    PIC1D_DBG_TILE_W = 9   /* int32 per tile of the last sort: width (sort cells) of the tile's key window */
 };
 int pic1d_debug_count(pic1d_t* h, int what, int species, int64_t* count_out);
 int pic1d_debug_get(pic1d_t* h, int what, int species, void* dst, size_t bytes);

@@ -243,7 +243,7 @@ void setup_launch(pic1d* h) {
     cudaFuncSetAttribute(k_field_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, FIELD_SMEM_MAX * (int)sizeof(double));
     cudaFuncSetAttribute(k_mcc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
-    h->WA = std::min((h->n_sc + 1 + 3) / 4 * 4, 1024);
+    h->WA = std::min((h->n_sc + 1 + 3) / 4 * 4, PIC1D_WA_MAX);
     h->smem_sort = (size_t)h->WA * sizeof(int);
     h->k_count = count_kernel(h->cfg.bc, h->T);
     h->grid_count = occupancy_grid(h, h->k_count, h->smem_sort);
@@ -597,6 +597,7 @@ int pic1d_debug_count(pic1d_t* h, int what, int s, int64_t* count_out) {
         case PIC1D_DBG_OFFSETS: *count_out = h->n_sc + 1; break;
         case PIC1D_DBG_MASK: *count_out = st.sp[s].n_sorted; break;
         case PIC1D_DBG_E32: case PIC1D_DBG_RHO_S: *count_out = h->nodes; break;
+        case PIC1D_DBG_TILE_W: *count_out = st.sp[s].n_tiles; break;
         default: return PIC1D_ERR_ARG;
     }
     return PIC1D_OK;
@@ -617,6 +618,7 @@ int pic1d_debug_get(pic1d_t* h, int what, int s, void* dst, size_t bytes) {
         case PIC1D_DBG_MASK: src = p.mask; el = 1; break;
         case PIC1D_DBG_E32: src = h->E32; break;
         case PIC1D_DBG_RHO_S: src = p.rho_s; el = 8; break;
+        case PIC1D_DBG_TILE_W: src = p.tile_w; break;
     }
     if (!src || bytes < (size_t)n * el) return PIC1D_ERR_ARG;
     if (n > 0 && !ck(h, cudaMemcpyAsync(dst, src, (size_t)n * el, cudaMemcpyDeviceToHost, h->stream))) return PIC1D_ERR_CUDA;

@@ -8,6 +8,7 @@
 
 #define PIC1D_NT 256          // threads per block of the particle kernels
 #define PIC1D_NWARP (PIC1D_NT / 32)
+#define PIC1D_WA_MAX 1024     // bins of a tile window ranked at a time in shared memory (multiple of 4)
 #define PIC1D_GROUP 64        // tiles per tile-group (window union used by the bin scan)
 
 // Philox stream ids (R12)

@@ -462,8 +462,8 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
             // direct: base = absolute destination; staged: base = position in the tile-sorted order,
             // and s_base becomes (absolute destination - position of the bin's first particle)
             unsigned n_out = 0;
-            {
-                const int i4 = tid * 4;
+            for (int c0 = 0; c0 < nsub; c0 += 4 * PIC1D_NT) {  // 1024 bins per round, in bin order
+                const int i4 = c0 + tid * 4;
                 const bool act = i4 < nsub;
                 uint4 tot = make_uint4(0u, 0u, 0u, 0u);
                 if (act) {
@@ -483,13 +483,14 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
                         const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
                         if (lane >= o) inc += t;
                     }
+                    if (c0 > 0) __syncthreads();  // s_scan of the previous round has been read
                     if (lane == 31) s_scan[wp] = inc;
                     __syncthreads();
                     unsigned before = 0, all = 0;
 #pragma unroll
                     for (int q = 0; q < PIC1D_NWARP; ++q) { const unsigned v = s_scan[q]; if (q < wp) before += v; all += v; }
-                    n_out = all;
-                    const unsigned e0 = before + inc - S;
+                    const unsigned e0 = n_out + before + inc - S;
+                    n_out += all;
                     const uint4 ls = make_uint4(e0, e0 + tot.x, e0 + tot.x + tot.y, e0 + tot.x + tot.y + tot.z);
                     if (act)
                         *reinterpret_cast<uint4*>(s_base + i4) = make_uint4(b4.x - ls.x, b4.y - ls.y, b4.z - ls.z, b4.w - ls.w);
@@ -539,8 +540,7 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
             __syncthreads();
             // ---- zero the counters again; next sub-window's bases ---------------------------------------
             {
-                const int i4 = tid * 4;
-                if (i4 < nsub) {
+                for (int i4 = tid * 4; i4 < nsub; i4 += 4 * PIC1D_NT) {
 #pragma unroll
                     for (int q = 0; q < PIC1D_NWARP; ++q)
                         *reinterpret_cast<uint4*>(s_cnt + q * WA + i4) = make_uint4(0u, 0u, 0u, 0u);
