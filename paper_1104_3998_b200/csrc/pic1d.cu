@@ -15,6 +15,7 @@
 #include "../../include/pic1d.h"
 #include "pic1d_device.cuh"
 #include "pic1d_sort.cuh"
+#include "pic1d_sort_warp.cuh"
 #include "pic1d_grid.cuh"
 #include "pic1d_mcc.cuh"
 
@@ -24,6 +25,8 @@ struct SpeciesHost {
     float* buf[2][4];
     int cur;
     int capacity, n_tiles_max, n_groups_max;
+    int T;            // slots per sort tile: 2048 / 1024 (block tiles) or PIC1D_TW (warp tiles)
+    bool warp_tiles;  // the species obeys Eq. 5: barrier-free warp-tile kernels (pic1d_sort_warp.cuh)
     int *tile_lo, *tile_w, *tile_off, *tile_dead, *grp_lo, *grp_hi, *pool;
     int pool_size, pool_stride, pool_fixed;
     int *hist, *offsets, *keys_dbg;
@@ -59,9 +62,9 @@ struct pic1d {
     bool ready;
     int64_t launches;
     cudaError_t last_err;
-    int grid_count, grid_scatter[2], WA;
-    size_t smem_sort, smem_scatter[2];
-    void (*k_count)(SortArgs);
+    int grid_count[2], grid_scatter[2], WA;
+    size_t smem_sort, smem_count[2], smem_scatter[2];
+    void (*k_count[2])(SortArgs);
     void (*k_scatter[2])(SortArgs);
     bool timing;
     std::vector<TimeMark> marks;
@@ -144,7 +147,9 @@ size_t layout(pic1d* h, char* base) {
         p.cur = 0;
         for (int b = 0; b < 2; ++b)
             for (int k = 0; k < 4; ++k) p.buf[b][k] = carve<float>(base, off, p.capacity);
-        p.n_tiles_max = p.capacity / h->T;
+        p.warp_tiles = s != 0;  // ions; electrons may move many cells per step (configs 2-4)
+        p.T = p.warp_tiles ? PIC1D_TW : h->T;
+        p.n_tiles_max = p.capacity / p.T;
         p.n_groups_max = (p.n_tiles_max + PIC1D_GROUP - 1) / PIC1D_GROUP;
         p.tile_lo = carve<int>(base, off, p.n_tiles_max);
         p.tile_w = carve<int>(base, off, p.n_tiles_max);
@@ -154,8 +159,8 @@ size_t layout(pic1d* h, char* base) {
         p.grp_hi = carve<int>(base, off, p.n_groups_max);
         // count pool: one fixed row of pool_stride bins per tile + an overflow region for wider windows
         const int64_t over = std::max<int64_t>(4 << 20, p.capacity / 4);
-        int64_t stride = std::min<int64_t>((h->n_sc + 3) / 4 * 4, 4096);
-        stride = std::max<int64_t>(4, std::min<int64_t>(stride, (((1ll << 31) - 1 - over) / p.n_tiles_max) / 4 * 4));
+        int64_t stride = p.warp_tiles ? PIC1D_PSW : std::min<int64_t>((h->n_sc + 3) / 4 * 4, 4096);
+        if (!p.warp_tiles) stride = std::max<int64_t>(4, std::min<int64_t>(stride, (((1ll << 31) - 1 - over) / p.n_tiles_max) / 4 * 4));
         p.pool_stride = (int)stride;
         p.pool_fixed = (int)(stride * p.n_tiles_max);
         p.pool_size = (int)(p.pool_fixed + over);
@@ -245,13 +250,23 @@ void setup_launch(pic1d* h) {
     cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     h->WA = std::min((h->n_sc + 1 + 3) / 4 * 4, PIC1D_WA_MAX);
     h->smem_sort = (size_t)h->WA * sizeof(int);
-    h->k_count = count_kernel(h->cfg.bc, h->T);
-    h->grid_count = occupancy_grid(h, h->k_count, h->smem_sort);
     for (int s = 0; s < h->cfg.n_species; ++s) {
+        SpeciesHost& p = h->sp[s];
         const bool abs = s == 1 && h->abs_list != nullptr;
-        const bool stage = s == 0;
-        h->k_scatter[s] = scatter_kernel(h->cfg.bc, h->T, abs, stage);
-        h->smem_scatter[s] = (size_t)h->WA * 9 * sizeof(unsigned) + (stage ? (size_t)h->T * 18 : 0);
+        if (p.warp_tiles) {
+            h->k_count[s] = h->cfg.bc == 1 ? k_push_count_w<1> : k_push_count_w<0>;
+            h->k_scatter[s] = h->cfg.bc == 1 ? k_push_scatter_w<1, false>
+                                             : (abs ? k_push_scatter_w<0, true> : k_push_scatter_w<0, false>);
+            h->smem_count[s] = 0;
+            h->smem_scatter[s] = 0;
+        } else {
+            const bool stage = s == 0;
+            h->k_count[s] = count_kernel(h->cfg.bc, h->T);
+            h->k_scatter[s] = scatter_kernel(h->cfg.bc, h->T, abs, stage);
+            h->smem_count[s] = h->smem_sort;
+            h->smem_scatter[s] = (size_t)h->WA * 9 * sizeof(unsigned) + (stage ? (size_t)h->T * 18 : 0);
+        }
+        h->grid_count[s] = occupancy_grid(h, h->k_count[s], h->smem_count[s]);
         h->grid_scatter[s] = occupancy_grid(h, h->k_scatter[s], h->smem_scatter[s]);
     }
 }
@@ -264,8 +279,10 @@ void enqueue_sort(pic1d* h, int s, int shift = 0) {
         a.shift = shift;
         a.n_sc = ((h->n_sc - 1) >> shift) + 1;
     }
-    const int gc = std::min(h->grid_count, p.n_tiles_max), gs = std::min(h->grid_scatter[s], p.n_tiles_max);
-    h->k_count<<<gc, PIC1D_NT, h->smem_sort, h->stream>>>(a);
+    const int tiles_per_block = p.warp_tiles ? PIC1D_NWARP : 1;
+    const int nb_max = (p.n_tiles_max + tiles_per_block - 1) / tiles_per_block;
+    const int gc = std::min(h->grid_count[s], nb_max), gs = std::min(h->grid_scatter[s], nb_max);
+    h->k_count[s]<<<gc, PIC1D_NT, h->smem_count[s], h->stream>>>(a);
     mark(h, "push_count", s);
     k_bin_scan<<<(a.n_sc + 31) / 32, BINSCAN_NW * 32, 0, h->stream>>>(a);
     mark(h, "bin_scan", s);
@@ -278,7 +295,7 @@ void enqueue_sort(pic1d* h, int s, int shift = 0) {
 
 void enqueue_begin(pic1d* h, int mode) {
     const int ns = h->cfg.n_species;
-    k_step_begin<<<4, 256, 0, h->stream>>>(h->st, ns, mode, h->T, h->sp[0].grp_lo, h->sp[0].grp_hi,
+    k_step_begin<<<4, 256, 0, h->stream>>>(h->st, ns, mode, h->sp[0].T, ns > 1 ? h->sp[1].T : 0, h->sp[0].grp_lo, h->sp[0].grp_hi,
                                            ns > 1 ? h->sp[1].grp_lo : nullptr, ns > 1 ? h->sp[1].grp_hi : nullptr,
                                            h->sp[0].n_groups_max, ns > 1 ? h->sp[1].n_groups_max : 0);
     mark(h, "step_begin", -1);
@@ -364,7 +381,7 @@ void enqueue_step(pic1d* h) {
             SeeArgs sa;
             sa.st = h->st; sa.abs_list = h->abs_list; sa.abs_cap = h->abs_cap;
             sa.ex = pe.buf[pe.cur][0]; sa.evx = pe.buf[pe.cur][1]; sa.evy = pe.buf[pe.cur][2]; sa.evz = pe.buf[pe.cur][3];
-            sa.cap_e = pe.capacity; sa.T = h->T;
+            sa.cap_e = pe.capacity; sa.T = pe.T;
             sa.gamma = (float)c.see_gamma; sa.vth = (float)c.see_vth; sa.fNc = (float)c.n_cells;
             sa.k0 = (uint32_t)c.seed; sa.k1 = (uint32_t)(c.seed >> 32); sa.step = h->step;
             k_see_emit<<<1, 1024, 0, h->stream>>>(sa);
@@ -483,19 +500,27 @@ int pic1d_load_particles(pic1d_t* h, int s, int64_t n, const float* x, const flo
         cudaMemsetAsync(pq.desc, 0, sizeof(ull) * pq.n_mcc_tiles, h->stream);
         if (pq.mask) cudaMemsetAsync(pq.mask, 0, pq.capacity, h->stream);
     }
-    // An unsorted load has full-width tile windows.  If the count pool cannot hold them, sort first
-    // by a coarse key (sort cell >> shift), then by the sort cell: two stable passes = one stable sort.
-    int shift = 0;
+    // An unsorted load has full-width tile windows, wider than a tile's fixed pool row.  Sort by the
+    // leading bits of the sort cell first, then by more bits, ... then by the sort cell: a sequence of
+    // stable passes = one stable sort, and every pass sees windows no wider than the pool row.
+    int bits = 0;
+    while ((1 << bits) < h->n_sc) ++bits;
+    int passes[PIC1D_MAX_SPECIES], sb[PIC1D_MAX_SPECIES], rounds = 1;
     for (int q = 0; q < h->cfg.n_species; ++q) {
-        const SpeciesHost& pq = h->sp[q];
-        while (((h->n_sc - 1) >> shift) + 1 > pq.pool_stride) ++shift;
+        sb[q] = 0;
+        while ((2 << sb[q]) <= h->sp[q].pool_stride) ++sb[q];
+        sb[q] = std::max(sb[q], 1);
+        passes[q] = std::max(1, (bits + sb[q] - 1) / sb[q]);
+        rounds = std::max(rounds, passes[q]);
     }
-    if (shift > 0) {
+    for (int r = 0; r < rounds; ++r) {
         enqueue_begin(h, 0);
-        for (int q = h->cfg.n_species - 1; q >= 0; --q) enqueue_sort(h, q, shift);
+        for (int q = h->cfg.n_species - 1; q >= 0; --q) {
+            const int pidx = r - (rounds - passes[q]);  // species with fewer passes join late
+            if (pidx < 0) continue;
+            enqueue_sort(h, q, std::max(0, bits - (pidx + 1) * sb[q]));
+        }
     }
-    enqueue_begin(h, 0);
-    for (int q = h->cfg.n_species - 1; q >= 0; --q) enqueue_sort(h, q);
     enqueue_grid(h, 0u);
     if (!ck(h, cudaGetLastError())) return PIC1D_ERR_CUDA;
     if (!on_device && !ck(h, cudaStreamSynchronize(h->stream))) return PIC1D_ERR_CUDA;  // host buffers may go away

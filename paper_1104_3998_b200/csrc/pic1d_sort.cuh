@@ -560,7 +560,7 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
 
 // ---- set up the sorts of one step ------------------------------------------------------------------
 // mode 0: initial sort after a load (nothing is pushed); mode 1: a regular step.
-__global__ void k_step_begin(DevState* st, int n_species, int mode, int T, int* grp_lo0, int* grp_hi0,
+__global__ void k_step_begin(DevState* st, int n_species, int mode, int T0, int T1, int* grp_lo0, int* grp_hi0,
                              int* grp_lo1, int* grp_hi1, int n_groups0, int n_groups1) {
     const int tid = threadIdx.x + blockIdx.x * blockDim.x;
     if (tid == 0) {
@@ -568,6 +568,7 @@ __global__ void k_step_begin(DevState* st, int n_species, int mode, int T, int* 
             DevSpecies& sp = st->sp[s];
             sp.n_push = mode ? sp.n_live : 0;
             sp.n_src = sp.n_live;
+            const int T = s == 0 ? T0 : T1;
             sp.n_tiles = (sp.n_live + T - 1) / T;
             sp.n_dead = 0;
             sp.pool_used = 0;

@@ -1,0 +1,239 @@
+// pic1d_sort_warp.cuh -- the fine sort for species that obey Eq. 5 ("only a small
+// number of particles leaves its sorting cell during one time step"): ions always, electrons of
+// Courant-respecting runs.
+//
+// Same two passes and the same pool / bin-scan bookkeeping as pic1d_sort.cuh, but a tile is the 256
+// consecutive slots ONE WARP owns, so no pass contains a block barrier: 32 independent warps per SM
+// stream through the particles and hide each other's latencies.
+//
+//   pass 1  k_push_count_w    x, vx -> push -> key; window [lo, hi] by redux; histogram of the warp's
+//                             256 keys in a 32-counter shared row (red.shared); fixed pool row of 32 bins
+//   pass 2  k_push_scatter_w  identical push; lane b keeps the next free destination of window bin b in
+//                             a shared row; per row of 32 slots: match.any groups equal keys, the lowest
+//                             lane of a group reads and advances the bin's cursor, the others take
+//                             cursor + (number of lower lanes with the same key).  Rows are taken in
+//                             slot order, so the sort is stable (R18) and no atomic is used.
+// Tiles whose window is wider than 32 bins (a species' birth tail, fast sheath ions) take a pool row
+// from the overflow region and keep their cursors in that row in global memory: slower, rare.
+#pragma once
+#include "pic1d_sort.cuh"
+
+#define PIC1D_TW 256  // slots per warp tile
+#define PIC1D_PSW 32  // bins of the fixed pool row of a warp tile (= warp size: lane b <-> window bin b)
+
+template <int BC>
+__global__ void __launch_bounds__(PIC1D_NT) k_push_count_w(SortArgs a) {
+    __shared__ int s_h[PIC1D_NWARP][PIC1D_PSW];
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    DevSpecies& sp = a.st->sp[a.s];
+    const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
+    const int n_warps = gridDim.x * PIC1D_NWARP;
+    for (int tile = blockIdx.x * PIC1D_NWARP + wp; tile < n_tiles; tile += n_warps) {
+        const int base = tile * PIC1D_TW;
+        int keys[8];
+        unsigned ulo = 0xffffffffu;
+        int hi = -1, smin = 0;
+        bool nonfinite = false;
+        const bool full = base + PIC1D_TW <= n_push && a.keys_dbg == nullptr;  // warp-uniform
+        if (full) {
+            float4 X[2], VX[2];
+#pragma unroll
+            for (int v = 0; v < 2; ++v) {
+                const int idx = base + v * 128 + lane * 4;
+                X[v] = __ldcs(reinterpret_cast<const float4*>(a.sx + idx));
+                VX[v] = __ldcs(reinterpret_cast<const float4*>(a.svx + idx));
+            }
+#pragma unroll
+            for (int v = 0; v < 2; ++v) {
+                float xs[4] = {X[v].x, X[v].y, X[v].z, X[v].w}, vs[4] = {VX[v].x, VX[v].y, VX[v].z, VX[v].w};
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int key = push_particle<BC>(xs[c], vs[c], true, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                    ulo = min(ulo, (unsigned)key); hi = max(hi, key); smin = min(smin, key);
+                    if (key == -2) nonfinite |= (xs[c] != xs[c]);
+                    keys[v * 4 + c] = key;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int v = 0; v < 2; ++v) {
+                const int idx = base + v * 128 + lane * 4;
+                float4 X = make_float4(0.f, 0.f, 0.f, 0.f), VX = X;
+                if (idx < n_src) {
+                    X = __ldcs(reinterpret_cast<const float4*>(a.sx + idx));
+                    VX = __ldcs(reinterpret_cast<const float4*>(a.svx + idx));
+                }
+                float xs[4] = {X.x, X.y, X.z, X.w}, vs[4] = {VX.x, VX.y, VX.z, VX.w};
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int i = idx + c;
+                    int key = -3;  // no particle
+                    smin = min(smin, i < n_src ? 0 : -3);
+                    if (i < n_src) {
+                        key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                        ulo = min(ulo, (unsigned)key); hi = max(hi, key); smin = min(smin, key);
+                        if (key == -2) nonfinite |= (xs[c] != xs[c]);
+                        if (a.keys_dbg) a.keys_dbg[i] = key >= 0 ? key : -1;
+                    }
+                    keys[v * 4 + c] = key;
+                }
+            }
+        }
+        ulo = __reduce_min_sync(0xffffffffu, ulo); hi = __reduce_max_sync(0xffffffffu, hi);
+        int lo = (int)ulo, dl = 0, dr = 0;
+        if (__any_sync(0xffffffffu, smin < 0)) {  // an absorbed or missing particle in the tile: rare
+            int lo2 = 0x7fffffff;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                dl += keys[q] == -1; dr += keys[q] == -2;
+                if (keys[q] >= 0) lo2 = min(lo2, keys[q]);
+            }
+            dl = __reduce_add_sync(0xffffffffu, dl); dr = __reduce_add_sync(0xffffffffu, dr);
+            lo = __reduce_min_sync(0xffffffffu, lo2);
+        }
+        if (nonfinite) atomicOr(&a.st->err, ERRBIT_NONFINITE);
+        const int w = hi >= 0 ? hi - lo + 1 : 0;
+        if (w == 0) lo = 0;
+        int off = tile * PIC1D_PSW;
+        if (w > PIC1D_PSW) {  // overflow region
+            int o = 0;
+            if (lane == 0) {
+                o = atomicAdd(&sp.pool_used, w);
+                if (o + w > a.pool_size - a.pool_fixed) { o = -1; atomicOr(&a.st->err, ERRBIT_WORKSPACE); }
+            }
+            o = __shfl_sync(0xffffffffu, o, 0);
+            off = o >= 0 ? a.pool_fixed + o : -1;
+        }
+        if (lane == 0) {
+            if (w > 0) {
+                atomicMin(&a.grp_lo[tile / PIC1D_GROUP], lo);
+                atomicMax(&a.grp_hi[tile / PIC1D_GROUP], hi);
+            }
+            a.tile_lo[tile] = lo; a.tile_w[tile] = off >= 0 ? w : 0; a.tile_off[tile] = off;
+            a.tile_dead[tile] = dl + dr;
+            if (dl) atomicAdd(&sp.absorbed_left, (ull)dl);
+            if (dr) atomicAdd(&sp.absorbed_right, (ull)dr);
+        }
+        // histogram of the warp's keys, 32 bins at a time (one round unless the window is wide)
+        for (int sub = 0; sub < w; sub += PIC1D_PSW) {
+            s_h[wp][lane] = 0;
+            __syncwarp();
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const unsigned r = (unsigned)(keys[q] - lo - sub);
+                if (r < (unsigned)PIC1D_PSW) atomicAdd(&s_h[wp][r], 1);
+            }
+            __syncwarp();
+            if (off >= 0 && sub + lane < w) a.pool[off + sub + lane] = s_h[wp][lane];
+            __syncwarp();
+        }
+    }
+}
+
+template <int BC, bool ABS>
+__global__ void __launch_bounds__(PIC1D_NT, 4) k_push_scatter_w(SortArgs a) {
+    __shared__ unsigned s_cur[PIC1D_NWARP][PIC1D_PSW + 1];  // next free destination per window bin (+ absorbed)
+    constexpr int ROWS = PIC1D_TW / 32;
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    DevSpecies& sp = a.st->sp[a.s];
+    const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
+    const int n_warps = gridDim.x * PIC1D_NWARP;
+    unsigned* cur = s_cur[wp];
+    for (int tile = blockIdx.x * PIC1D_NWARP + wp; tile < n_tiles; tile += n_warps) {
+        const int lo = a.tile_lo[tile], w = a.tile_w[tile], off = a.tile_off[tile];
+        if (off < 0) continue;  // count pool exhausted (sticky error): drop the tile
+        const int base = tile * PIC1D_TW + lane;
+        const bool full = tile * PIC1D_TW + PIC1D_TW <= n_push;  // warp-uniform
+        const bool narrow = w <= PIC1D_PSW;
+        float x[ROWS], vx[ROWS], vy[ROWS], vz[ROWS];
+        int k[ROWS];  // bin relative to the window; w = absorbed (ABS); -1 = no particle
+        unsigned wall = 0;
+        if (full) {
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) { x[r] = __ldcs(a.sx + base + r * 32); vx[r] = __ldcs(a.svx + base + r * 32); }
+        } else {
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) {
+                const int i = base + r * 32;
+                x[r] = 0.0f; vx[r] = 0.0f;
+                if (i < n_src) { x[r] = __ldcs(a.sx + i); vx[r] = __ldcs(a.svx + i); }
+            }
+        }
+        // cursors of the window bins: first destination of this tile's particles per bin
+        unsigned c0 = 0;
+        if (narrow && lane < w) c0 = (unsigned)(a.offsets[lo + lane] + __ldcg(a.pool + off + lane));
+        unsigned cdead = 0;
+        if (ABS) cdead = (unsigned)a.tile_dead[tile];
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r) {
+            const int i = base + r * 32;
+            k[r] = -1;
+            if (full || i < n_src) {
+                const int key = push_particle<BC>(x[r], vx[r], full || i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                k[r] = key >= 0 ? key - lo : (ABS ? w : -1);
+                if (ABS && key == -2) wall |= 1u << r;
+            }
+        }
+        if (full) {
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) { vy[r] = __ldcs(a.svy + base + r * 32); vz[r] = __ldcs(a.svz + base + r * 32); }
+        } else {
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) {
+                const int i = base + r * 32;
+                vy[r] = 0.0f; vz[r] = 0.0f;
+                if (i < n_src) { vy[r] = __ldcs(a.svy + i); vz[r] = __ldcs(a.svz + i); }
+            }
+        }
+        __syncwarp();  // the previous tile's rows are done with the cursors
+        if (narrow) {
+            cur[lane] = lane < w ? c0 : cdead;     // bin w (the absorbed pseudo-bin, ABS) follows the window
+            if (lane == 0) cur[PIC1D_PSW] = cdead;  // ... also when the window has all 32 bins
+            __syncwarp();
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) {
+                const int kk = k[r];
+                const unsigned peers = __match_any_sync(0xffffffffu, kk);
+                const int leader = __ffs(peers) - 1;
+                unsigned old = 0;
+                if (kk >= 0 && lane == leader) { old = cur[kk]; cur[kk] = old + __popc(peers); }
+                old = __shfl_sync(0xffffffffu, old, leader);
+                const unsigned d = old + __popc(peers & lanemask_lt());
+                if (kk >= 0) {
+                    if (!ABS || kk < w) {
+                        a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
+                    } else if (a.abs_list && (int)d < a.abs_cap) {  // absorbed: ordered list of (slot, wall)
+                        a.abs_list[d] = (unsigned)(base + r * 32) | (((wall >> r) & 1u) << 31);
+                    }
+                }
+                __syncwarp();  // the next row's leaders see the advanced cursors
+            }
+        } else {
+            // wide window: the cursors stay in the tile's pool row (exclusive prefixes over earlier tiles)
+            if (ABS && lane == 0) cur[0] = cdead;
+            __syncwarp();
+            volatile int* row = a.pool + off;
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) {
+                const int kk = k[r];
+                const unsigned peers = __match_any_sync(0xffffffffu, kk);
+                const int leader = __ffs(peers) - 1;
+                unsigned old = 0;
+                if (kk >= 0 && lane == leader) {
+                    if (!ABS || kk < w) { old = (unsigned)row[kk]; row[kk] = (int)(old + __popc(peers)); old += (unsigned)a.offsets[lo + kk]; }
+                    else { old = cur[0]; cur[0] = old + __popc(peers); }
+                }
+                old = __shfl_sync(0xffffffffu, old, leader);
+                const unsigned d = old + __popc(peers & lanemask_lt());
+                if (kk >= 0) {
+                    if (!ABS || kk < w) {
+                        a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
+                    } else if (a.abs_list && (int)d < a.abs_cap) {
+                        a.abs_list[d] = (unsigned)(base + r * 32) | (((wall >> r) & 1u) << 31);
+                    }
+                }
+                __syncwarp();
+            }
+        }
+    }
+}
