@@ -284,7 +284,7 @@ void enqueue_sort(pic1d* h, int s, int shift = 0) {
     const int gc = std::min(h->grid_count[s], nb_max), gs = std::min(h->grid_scatter[s], nb_max);
     h->k_count[s]<<<gc, PIC1D_NT, h->smem_count[s], h->stream>>>(a);
     mark(h, "push_count", s);
-    k_bin_scan<<<(a.n_sc + 31) / 32, BINSCAN_NW * 32, 0, h->stream>>>(a);
+    k_bin_scan<<<(a.n_sc + 31) / 32 + (a.abs_list ? 1 : 0), BINSCAN_NW * 32, 0, h->stream>>>(a);
     mark(h, "bin_scan", s);
     k_offsets_scan<<<1, 1024, 0, h->stream>>>(a);
     mark(h, "offsets_scan", s);

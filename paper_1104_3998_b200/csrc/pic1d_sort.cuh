@@ -184,6 +184,63 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
     }
 }
 
+// block-wide exclusive scan of src[0..n) into dst[0..n), returns the total; single block, any n.
+// Every warp owns a contiguous segment and walks it in rows of 32 (coalesced): pass 1 sums the
+// segment (independent loads), a shuffle scan orders the warps, pass 2 scans row by row with a carry.
+// dst may alias src.
+// SPARSE: rows of 32 zeros are skipped (their dst entries are NOT written: callers only read the
+// prefix at positions whose src was non-zero).
+template <bool SPARSE = false>
+__device__ int block_exclusive_scan(const int* src, int* dst, int n) {
+    __shared__ int s_w[33];
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5, nw = blockDim.x >> 5;
+    const int seg = ((n + nw * 32 - 1) / (nw * 32)) * 32;  // elements per warp, a multiple of 32
+    const int b = min(wp * seg, n), e = min(b + seg, n);
+    int tot = 0;
+    for (int i = b + lane; i < e; i += 32 * 8) {
+        int v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = i + u * 32 < e ? src[i + u * 32] : 0;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) tot += v[u];
+    }
+    tot = __reduce_add_sync(0xffffffffu, tot);
+    __syncthreads();  // s_w may still be read by a previous call
+    if (lane == 0) s_w[wp] = tot;
+    __syncthreads();
+    if (wp == 0) {
+        const int t = lane < nw ? s_w[lane] : 0;
+        int ti = t;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int u = __shfl_up_sync(0xffffffffu, ti, o);
+            if (lane >= o) ti += u;
+        }
+        s_w[lane] = ti - t;  // exclusive over warps
+        if (lane == 31) s_w[32] = ti;
+    }
+    __syncthreads();
+    int carry = s_w[wp];
+    for (int i0 = b; i0 < e; i0 += 32 * 4) {
+        int v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = i0 + u * 32 + lane < e ? src[i0 + u * 32 + lane] : 0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (SPARSE && !__any_sync(0xffffffffu, v[u] != 0)) continue;
+            int inc = v[u];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            if (i0 + u * 32 + lane < e) dst[i0 + u * 32 + lane] = carry + inc - v[u];
+            carry += __shfl_sync(0xffffffffu, inc, 31);
+        }
+    }
+    return s_w[32];
+}
+
 // ---- scan over tiles, per sort cell --------------------------------------------------------------
 // Block = 32 adjacent sort cells (lane = cell k) x 32 warps.  The tiles whose window can contain the
 // block's cells form a short range [ta, tb) (found from the tile-group windows); it is split evenly
@@ -197,25 +254,43 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
     __shared__ unsigned short s_list[BINSCAN_LIST];  // tile groups whose window overlaps the block's cells
     __shared__ int s_part[BINSCAN_NW][33];
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    if (blockIdx.x * 32 >= a.n_sc) {
+        // one extra block (species with an ordered absorbed list only): exclusive prefix of the per-tile
+        // absorbed counts, concurrently with the bin blocks
+        DevSpecies& sp = a.st->sp[a.s];
+        const int n_dead = block_exclusive_scan<true>(a.tile_dead, a.tile_dead, sp.n_tiles);
+        if (tid == 0) sp.n_dead = n_dead;
+        return;
+    }
     const int kb0 = blockIdx.x * 32, kb1 = min(kb0 + 31, a.n_sc - 1);
     const int k = kb0 + lane;
     const int n_tiles = a.st->sp[a.s].n_tiles;
     const int n_groups = (n_tiles + PIC1D_GROUP - 1) / PIC1D_GROUP;
     // ordered list of the relevant groups (a group is skipped as a whole: the birth tail of a species
-    // has full-width windows and must not drag every tile before it into the walk)
+    // has full-width windows and must not drag every tile before it into the walk).  Thread t owns the
+    // contiguous chunk of groups [t gpt, (t+1) gpt): count, block-wide exclusive scan, write.
     int n_rel = 0;
-    for (int g0 = 0; g0 < n_groups; g0 += BINSCAN_NW * 32) {
-        const int g = g0 + tid;
-        const bool rel = g < n_groups && a.grp_hi[g] >= kb0 && a.grp_lo[g] <= kb1;
-        const unsigned bal = __ballot_sync(0xffffffffu, rel);
-        if (lane == 0) s_wc[wp] = __popc(bal);
+    {
+        const int gpt = (n_groups + BINSCAN_NW * 32 - 1) / (BINSCAN_NW * 32);
+        const int g_beg = min(tid * gpt, n_groups), g_end = min(g_beg + gpt, n_groups);
+        int mine = 0;
+        for (int g = g_beg; g < g_end; ++g) mine += (a.grp_hi[g] >= kb0 && a.grp_lo[g] <= kb1) ? 1 : 0;
+        int inc = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) s_wc[wp] = inc;
         __syncthreads();
-        int before = 0, tot = 0;
+        int before = 0;
 #pragma unroll 8
-        for (int q = 0; q < BINSCAN_NW; ++q) { const int v = s_wc[q]; if (q < wp) before += v; tot += v; }
-        const int idx = n_rel + before + __popc(bal & lanemask_lt());
-        if (rel && idx < BINSCAN_LIST) s_list[idx] = (unsigned short)g;
-        n_rel += tot;
+        for (int q = 0; q < BINSCAN_NW; ++q) { const int v = s_wc[q]; if (q < wp) before += v; n_rel += v; }
+        int idx = before + inc - mine;
+        if (mine) {
+            for (int g = g_beg; g < g_end; ++g)
+                if (a.grp_hi[g] >= kb0 && a.grp_lo[g] <= kb1) { if (idx < BINSCAN_LIST) s_list[idx] = (unsigned short)g; ++idx; }
+        }
         __syncthreads();
     }
     // n_rel groups (or, if the list overflowed, every group) -> virtual tile range split over the warps
@@ -275,71 +350,14 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
     if (wp == 0 && k < a.n_sc) a.hist[k] = total;
 }
 
-// block-wide exclusive scan of src[0..n) into dst[0..n), returns the total; single block, any n.
-// Every warp owns a contiguous segment and walks it in rows of 32 (coalesced): pass 1 sums the
-// segment (independent loads), a shuffle scan orders the warps, pass 2 scans row by row with a carry.
-// dst may alias src.
-__device__ int block_exclusive_scan(const int* src, int* dst, int n) {
-    __shared__ int s_w[33];
-    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5, nw = blockDim.x >> 5;
-    const int seg = ((n + nw * 32 - 1) / (nw * 32)) * 32;  // elements per warp, a multiple of 32
-    const int b = min(wp * seg, n), e = min(b + seg, n);
-    int tot = 0;
-    for (int i = b + lane; i < e; i += 32 * 8) {
-        int v[8];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) v[u] = i + u * 32 < e ? src[i + u * 32] : 0;
-#pragma unroll
-        for (int u = 0; u < 8; ++u) tot += v[u];
-    }
-    tot = __reduce_add_sync(0xffffffffu, tot);
-    __syncthreads();  // s_w may still be read by a previous call
-    if (lane == 0) s_w[wp] = tot;
-    __syncthreads();
-    if (wp == 0) {
-        const int t = lane < nw ? s_w[lane] : 0;
-        int ti = t;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int u = __shfl_up_sync(0xffffffffu, ti, o);
-            if (lane >= o) ti += u;
-        }
-        s_w[lane] = ti - t;  // exclusive over warps
-        if (lane == 31) s_w[32] = ti;
-    }
-    __syncthreads();
-    int carry = s_w[wp];
-    for (int i0 = b; i0 < e; i0 += 32 * 4) {
-        int v[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) v[u] = i0 + u * 32 + lane < e ? src[i0 + u * 32 + lane] : 0;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            int inc = v[u];
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int t = __shfl_up_sync(0xffffffffu, inc, o);
-                if (lane >= o) inc += t;
-            }
-            if (i0 + u * 32 + lane < e) dst[i0 + u * 32 + lane] = carry + inc - v[u];
-            carry += __shfl_sync(0xffffffffu, inc, 31);
-        }
-    }
-    return s_w[32];
-}
-
-// offsets[k] = #{key < k}; n_live = n_sorted = survivors; exclusive prefix of absorbed counts (only
-// needed when the species keeps an ordered absorbed list).
+// offsets[k] = #{key < k}; n_live = n_sorted = survivors.
 __global__ void __launch_bounds__(1024) k_offsets_scan(SortArgs a) {
     DevSpecies& sp = a.st->sp[a.s];
-    const int total = block_exclusive_scan(a.hist, a.offsets, a.n_sc);
-    int n_dead = 0;
-    if (a.abs_list) n_dead = block_exclusive_scan(a.tile_dead, a.tile_dead, sp.n_tiles);
+    const int total = block_exclusive_scan<false>(a.hist, a.offsets, a.n_sc);
     if (threadIdx.x == 0) {
         a.offsets[a.n_sc] = total;
         sp.n_live = total;
         sp.n_sorted = total;
-        sp.n_dead = n_dead;
     }
 }
 

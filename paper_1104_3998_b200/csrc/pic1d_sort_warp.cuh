@@ -114,18 +114,26 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count_w(SortArgs a) {
             if (dl) atomicAdd(&sp.absorbed_left, (ull)dl);
             if (dr) atomicAdd(&sp.absorbed_right, (ull)dr);
         }
-        // histogram of the warp's keys, 32 bins at a time (one round unless the window is wide)
-        for (int sub = 0; sub < w; sub += PIC1D_PSW) {
+        if (w <= PIC1D_PSW) {
+            // histogram of the warp's keys in a 32-counter shared row
             s_h[wp][lane] = 0;
             __syncwarp();
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-                const unsigned r = (unsigned)(keys[q] - lo - sub);
+                const unsigned r = (unsigned)(keys[q] - lo);
                 if (r < (unsigned)PIC1D_PSW) atomicAdd(&s_h[wp][r], 1);
             }
             __syncwarp();
-            if (off >= 0 && sub + lane < w) a.pool[off + sub + lane] = s_h[wp][lane];
+            if (lane < w) a.pool[off + lane] = s_h[wp][lane];
             __syncwarp();
+        } else if (off >= 0) {
+            // wide window (rare): zero the tile's overflow row, then count straight into it
+            for (int i = lane; i < w; i += 32) a.pool[off + i] = 0;
+            __threadfence();
+            __syncwarp();
+#pragma unroll
+            for (int q = 0; q < 8; ++q)
+                if (keys[q] >= 0) atomicAdd(&a.pool[off + keys[q] - lo], 1);
         }
     }
 }
