@@ -92,11 +92,13 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
         if (tile >= n_act) break;
         const int tbase = tile * MCC_TILE;
         // ---- phase A: null test, 4 slots per Philox call ------------------------------------------
+        constexpr int NQ = MCC_TILE / (4 * PIC1D_NT);  // quads per thread
+        const bool tile_full = tbase + MCC_TILE <= n_sorted;  // block-uniform
+        unsigned bits = 0;  // bit 4 q + c: slot c of the thread's quad q is a candidate
 #pragma unroll
-        for (int q = 0; q < MCC_TILE / (4 * PIC1D_NT); ++q) {
+        for (int q = 0; q < NQ; ++q) {
             const int rel0 = (q * PIC1D_NT + tid) * 4, i0 = tbase + rel0;
-            unsigned bits = 0;
-            if (i0 < n_sorted) {
+            if (tile_full || i0 < n_sorted) {
                 float4 A, B, C;
                 if (STAGE) {  // buffers have capacity slots (a multiple of 4096): the vector never leaves them
                     A = *reinterpret_cast<const float4*>(a.vx + i0);
@@ -107,8 +109,7 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
                 philox4x32_10((uint32_t)(i0 >> 2), a.step, str_null, 0u, a.k0, a.k1, w);
 #pragma unroll
                 for (int c = 0; c < 4; ++c)
-                    if (i0 + c < n_sorted && w[c] <= a.null_le) bits |= 1u << c;
-                if (!a.null_any) bits = 0;
+                    if ((tile_full || i0 + c < n_sorted) && w[c] <= a.null_le) bits |= 1u << (4 * q + c);
                 if (a.mask) *reinterpret_cast<uchar4*>(a.mask + i0) = make_uchar4(0, 0, 0, 0);  // 4-aligned, capacity slots
                 if (STAGE) {
                     *reinterpret_cast<float4*>(s_vx + rel0) = A;
@@ -116,7 +117,10 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
                     *reinterpret_cast<float4*>(s_vz + rel0) = C;
                 }
             }
-            // ordered append: exclusive prefix of the per-thread counts inside the warp
+        }
+        if (!a.null_any) bits = 0;
+        {
+            // append the thread's candidates to the shared list (any order: each is handled on its own)
             const int cnt = __popc(bits);
             int inc = cnt;
 #pragma unroll
@@ -127,9 +131,17 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
             int base = 0;
             if (lane == 31 && inc) base = atomicAdd(&s_n[0], inc);
             base = __shfl_sync(0xffffffffu, base, 31) + inc - cnt;
+            if (STAGE) {  // most slots are candidates: predicated stores
 #pragma unroll
-            for (int c = 0; c < 4; ++c)
-                if ((bits >> c) & 1u) s_cand[base++] = (unsigned short)(rel0 + c);
+                for (int b = 0; b < 4 * NQ; ++b)
+                    if ((bits >> b) & 1u) s_cand[base++] = (unsigned short)(((b >> 2) * PIC1D_NT + tid) * 4 + (b & 3));
+            } else {      // few are: walk the set bits
+                while (bits) {
+                    const int b = __ffs(bits) - 1;
+                    bits &= bits - 1;
+                    s_cand[base++] = (unsigned short)(((b >> 2) * PIC1D_NT + tid) * 4 + (b & 3));
+                }
+            }
         }
         __syncthreads();
         // ---- phase B: process selection, one thread per candidate ----------------------------------
@@ -152,14 +164,23 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
                 const float aa = __fmul_rn(g, a.inv_g_cap);
                 if (aa > 1.0f) ++c_over;
                 if (KIND == 1) {
+                    // cumulative selection, evaluated lazily: the same operations as the full form,
+                    // only skipped where their result cannot matter (P_exc = P_ion = 0 below E_exc)
                     const float En = __fmul_rn(a.c_eV, g2);
-                    const float P_el = __fmul_rn(aa, a.r_el);
-                    const float P_exc = En > a.E_exc
-                        ? __fmul_rn(__fmul_rn(aa, a.r_exc), __fsub_rn(1.0f, __fdiv_rn(a.E_exc, En))) : 0.0f;
-                    const float P_ion = En > a.E_ion
-                        ? __fmul_rn(__fmul_rn(aa, a.r_ion), __fsub_rn(1.0f, __fdiv_rn(a.E_ion, En))) : 0.0f;
-                    const float t1 = P_el, t2 = __fadd_rn(t1, P_exc), t3 = __fadd_rn(t2, P_ion);
-                    e = u_type < t1 ? 1 : (u_type < t2 ? 2 : (u_type < t3 ? 3 : 0));
+                    const float t1 = __fmul_rn(aa, a.r_el);
+                    if (u_type < t1) {
+                        e = 1;
+                    } else if (En > a.E_exc) {
+                        const float P_exc = __fmul_rn(__fmul_rn(aa, a.r_exc), __fsub_rn(1.0f, __fdiv_rn(a.E_exc, En)));
+                        const float t2 = __fadd_rn(t1, P_exc);
+                        if (u_type < t2) {
+                            e = 2;
+                        } else {
+                            const float P_ion = En > a.E_ion
+                                ? __fmul_rn(__fmul_rn(aa, a.r_ion), __fsub_rn(1.0f, __fdiv_rn(a.E_ion, En))) : 0.0f;
+                            e = u_type < __fadd_rn(t2, P_ion) ? 3 : 0;
+                        }
+                    }
                 } else {  // ion charge exchange with the cold background gas
                     e = u_type < fminf(1.0f, aa) ? 1 : 0;
                 }
@@ -169,7 +190,7 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
             }
             const int idx = warp_append(e != 0, &s_n[1]);
             if (e) s_coll[idx] = (unsigned short)(rel | (e << 12));
-            warp_append(e == 3, &s_n[2]);
+            if (KIND == 1 && __any_sync(0xffffffffu, e == 3)) warp_append(e == 3, &s_n[2]);
         }
         c_e0 += c_pack & 0xff; c_e1 += (c_pack >> 8) & 0xff; c_e2 += (c_pack >> 16) & 0xff; c_e3 += c_pack >> 24;
         __syncthreads();
