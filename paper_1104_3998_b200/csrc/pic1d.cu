@@ -176,7 +176,7 @@ size_t layout(pic1d* h, char* base) {
         p.part = carve<double>(base, off, (size_t)h->n_dep_blocks * h->G);
         p.side = carve<double>(base, off, h->n_dep_blocks);
         p.rho_s = carve<double>(base, off, h->nodes + 1);
-        p.n_mcc_tiles = (p.capacity + MCC_TILE - 1) / MCC_TILE;
+        p.n_mcc_tiles = (p.capacity + MCC_TILE_STAGE - 1) / MCC_TILE_STAGE;
         p.desc = carve<ull>(base, off, p.n_mcc_tiles);
     }
     return align_up(off, 256);
@@ -246,8 +246,8 @@ int occupancy_grid(pic1d* h, sort_kernel_t kernel, size_t smem) {
 
 void setup_launch(pic1d* h) {
     cudaFuncSetAttribute(k_field_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, FIELD_SMEM_MAX * (int)sizeof(double));
-    cudaFuncSetAttribute(k_mcc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
-    cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
+    cudaFuncSetAttribute(k_mcc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE_STAGE * sizeof(float)));
+    cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE_STAGE * sizeof(float)));
     h->WA = std::min((h->n_sc + 1 + 3) / 4 * 4, PIC1D_WA_MAX);
     h->smem_sort = (size_t)h->WA * sizeof(int);
     for (int s = 0; s < h->cfg.n_species; ++s) {
@@ -361,10 +361,10 @@ void enqueue_mcc(pic1d* h) {
         const int grid = std::min(p.n_mcc_tiles, h->num_sms * 4);
         const bool stage = c.sp[s].P0 > 0.25;
         if (m.kind == 1) {
-            if (stage) k_mcc<1, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE * sizeof(float), h->stream>>>(m);
+            if (stage) k_mcc<1, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE_STAGE * sizeof(float), h->stream>>>(m);
             else k_mcc<1, false><<<grid, PIC1D_NT, MCC_TILE * sizeof(float), h->stream>>>(m);
         } else {
-            if (stage) k_mcc<2, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE * sizeof(float), h->stream>>>(m);
+            if (stage) k_mcc<2, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE_STAGE * sizeof(float), h->stream>>>(m);
             else k_mcc<2, false><<<grid, PIC1D_NT, 0, h->stream>>>(m);
         }
         mark(h, "mcc", s);

@@ -19,7 +19,8 @@
 #pragma once
 #include "pic1d_device.cuh"
 
-#define MCC_TILE (PIC1D_NT * 16)
+#define MCC_TILE (PIC1D_NT * 16)       // sorted slots per tile
+#define MCC_TILE_STAGE (PIC1D_NT * 16) // ... when the velocities are staged in shared memory (8: slower)
 
 struct MccArgs {
     float *x, *vx, *vy, *vz;      // this species' current (sorted) buffer
@@ -67,33 +68,34 @@ __device__ __forceinline__ int warp_append(bool flag, int* counter) {
 // otherwise phases B / C fetch the few candidates' velocities from global memory.
 template <int KIND, bool STAGE>
 __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
-    extern __shared__ float s_v[];  // STAGE: [3][MCC_TILE] velocities; else (KIND 1): [MCC_TILE] speeds of ionising slots
+    constexpr int TILE = STAGE ? MCC_TILE_STAGE : MCC_TILE;
+    extern __shared__ float s_v[];  // STAGE: [3][TILE] velocities; else (KIND 1): [TILE] speeds of ionising slots
     __shared__ int s_tile, s_excl;
     __shared__ int s_n[3];                          // candidates, real collisions, ionisations
-    __shared__ unsigned short s_cand[MCC_TILE];     // slot - tile base
-    __shared__ unsigned short s_coll[MCC_TILE];     // (slot - tile base) | event << 12
-    __shared__ unsigned s_ionbits[MCC_TILE / 32];   // bit = slot ionises
+    __shared__ unsigned short s_cand[TILE];     // slot - tile base
+    __shared__ unsigned short s_coll[TILE];     // (slot - tile base) | event << 12
+    __shared__ unsigned s_ionbits[TILE / 32];   // bit = slot ionises
     const int tid = threadIdx.x, lane = tid & 31;
     DevState* st = a.st;
     DevSpecies& sp = st->sp[a.s];
     const int n_sorted = sp.n_sorted;
-    const int n_act = (n_sorted + MCC_TILE - 1) / MCC_TILE;
+    const int n_act = (n_sorted + TILE - 1) / TILE;
     const uint32_t epoch = a.step + 1u;
     const uint32_t str_null = STREAM_NULL + (uint32_t)a.s, str_coll = STREAM_COLL + (uint32_t)a.s;
     int c_cand = 0, c_e0 = 0, c_e1 = 0, c_e2 = 0, c_e3 = 0, c_over = 0;
-    float* s_vx = s_v; float* s_vy = s_v + MCC_TILE; float* s_vz = s_v + 2 * MCC_TILE;
+    float* s_vx = s_v; float* s_vy = s_v + TILE; float* s_vz = s_v + 2 * TILE;
     unsigned short* s_ion_rel = s_cand;  // ionising slots in slot order (the candidate list is dead by then)
     float* s_gp = s_v;                   // [slot - tile base] speed shared by the two electrons (its vx is dead by then)
     while (true) {
         if (tid == 0) { s_tile = atomicAdd(&sp.ticket, 1); s_n[0] = 0; s_n[1] = 0; s_n[2] = 0; }
-        if (tid < MCC_TILE / 32) s_ionbits[tid] = 0u;
+        if (tid < TILE / 32) s_ionbits[tid] = 0u;
         __syncthreads();
         const int tile = s_tile;
         if (tile >= n_act) break;
-        const int tbase = tile * MCC_TILE;
+        const int tbase = tile * TILE;
         // ---- phase A: null test, 4 slots per Philox call ------------------------------------------
-        constexpr int NQ = MCC_TILE / (4 * PIC1D_NT);  // quads per thread
-        const bool tile_full = tbase + MCC_TILE <= n_sorted;  // block-uniform
+        constexpr int NQ = TILE / (4 * PIC1D_NT);  // quads per thread
+        const bool tile_full = tbase + TILE <= n_sorted;  // block-uniform
         unsigned bits = 0;  // bit 4 q + c: slot c of the thread's quad q is a candidate
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
@@ -194,12 +196,60 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
         }
         c_e0 += c_pack & 0xff; c_e1 += (c_pack >> 8) & 0xff; c_e2 += (c_pack >> 16) & 0xff; c_e3 += c_pack >> 24;
         __syncthreads();
-        // ---- publish this tile's ionisation count for the look-back of later tiles ---------------
+        // ---- ordered births: publish this tile's ionisation count, then the exclusive prefix over earlier
+        // tiles by a warp-wide decoupled look-back (32 predecessors per probe), while the other warps
+        // already run phase C ----------------------------------------------------------------------
         const int nb = s_n[2];
-        if (KIND == 1 && tid == 0) {
+        if (KIND == 1 && tid < 32) {
             volatile ull* desc = a.desc;
-            desc[tile] = desc_pack(epoch, tile == 0 ? DESC_PREFIX : DESC_AGG, nb);
-            __threadfence();
+            if (lane == 0) {
+                desc[tile] = desc_pack(epoch, tile == 0 ? DESC_PREFIX : DESC_AGG, nb);
+                __threadfence();
+            }
+            int excl = 0;
+            int j = tile - 1;  // this probe looks at tiles j, j-1, ..., j-31
+            while (j >= 0) {
+                const int idx = j - lane;
+                const ull d = idx >= 0 ? desc[idx] : desc_pack(epoch, DESC_PREFIX, 0);  // before tile 0: prefix 0
+                const bool ready = (uint32_t)(d >> 32) == epoch;
+                const bool is_p = ready && ((d >> 30) & 3ull) == DESC_PREFIX;
+                const unsigned nr = __ballot_sync(0xffffffffu, !ready), pm = __ballot_sync(0xffffffffu, is_p);
+                const int first_p = pm ? __ffs(pm) - 1 : 32, first_nr = nr ? __ffs(nr) - 1 : 32;
+                const int v = (int)(d & 0x3fffffffull);
+                if (first_p < first_nr) {         // a prefix, and everything nearer than it is published
+                    excl += __reduce_add_sync(0xffffffffu, lane <= first_p ? v : 0);
+                    break;
+                }
+                if (first_nr == 32) {             // 32 aggregates: take them all, look further back
+                    excl += __reduce_add_sync(0xffffffffu, v);
+                    j -= 32;
+                }                                 // else: somebody nearer than any prefix is not there yet: probe again
+            }
+            if (lane == 0) {
+                if (tile > 0) {
+                    desc[tile] = desc_pack(epoch, DESC_PREFIX, excl + nb);
+                    __threadfence();
+                }
+                s_excl = excl;
+                if (tile == n_act - 1) {  // last tile: close the step's birth bookkeeping
+                    const int total = excl + nb;
+                    const int ne = st->sp[0].n_sorted;
+                    int room = a.cap_e - ne;
+                    if (a.n_species > 1) room = min(room, a.cap_i - st->sp[1].n_sorted);
+                    const int kept = min(total, max(room, 0));
+                    st->sp[0].n_live = ne + kept;
+                    st->sp[0].births += (ull)kept;
+                    if (a.n_species > 1) {
+                        st->sp[1].n_live = st->sp[1].n_sorted + kept;
+                        st->sp[1].births += (ull)kept;
+                    }
+                    if (total > kept) {
+                        st->sp[0].dropped += (ull)(total - kept);
+                        if (a.n_species > 1) st->sp[1].dropped += (ull)(total - kept);
+                        atomicOr(&st->err, ERRBIT_CAPACITY);
+                    }
+                }
+            }
         }
         // ---- phase C: kinematics, one thread per real collision -------------------------------------
         const int n_coll = s_n[1];
@@ -243,42 +293,6 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
             }
         }
         if (KIND != 1) { __syncthreads(); continue; }
-        // ---- ordered births: exclusive prefix over earlier tiles by decoupled look-back --------------
-        if (tid == 0) {
-            volatile ull* desc = a.desc;
-            int excl = 0;
-            if (tile > 0) {
-                int j = tile - 1;
-                while (true) {
-                    const ull d = desc[j];
-                    if ((uint32_t)(d >> 32) != epoch) continue;  // not published yet this step
-                    excl += (int)(d & 0x3fffffffull);
-                    if (((d >> 30) & 3ull) == DESC_PREFIX) break;
-                    --j;
-                }
-                desc[tile] = desc_pack(epoch, DESC_PREFIX, excl + nb);
-                __threadfence();
-            }
-            s_excl = excl;
-            if (tile == n_act - 1) {  // last tile: close the step's birth bookkeeping
-                const int total = excl + nb;
-                const int ne = st->sp[0].n_sorted;
-                int room = a.cap_e - ne;
-                if (a.n_species > 1) room = min(room, a.cap_i - st->sp[1].n_sorted);
-                const int kept = min(total, max(room, 0));
-                st->sp[0].n_live = ne + kept;
-                st->sp[0].births += (ull)kept;
-                if (a.n_species > 1) {
-                    st->sp[1].n_live = st->sp[1].n_sorted + kept;
-                    st->sp[1].births += (ull)kept;
-                }
-                if (total > kept) {
-                    st->sp[0].dropped += (ull)(total - kept);
-                    if (a.n_species > 1) st->sp[1].dropped += (ull)(total - kept);
-                    atomicOr(&st->err, ERRBIT_CAPACITY);
-                }
-            }
-        }
         __syncthreads();
         // ---- phase D: one thread per ionisation: the new electron / ion pair -------------------------
         if (nb > 0) {
