@@ -249,10 +249,12 @@ __device__ int block_exclusive_scan(const int* src, int* dst, int n) {
 // (exclusive prefix over tiles); hist[k] gets the total.  Row segments of the pool are read coalesced.
 #define BINSCAN_NW 32
 #define BINSCAN_LIST 4096
+#define BINSCAN_DESC 2048  // tile descriptors a block can keep in shared memory
 __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
     __shared__ int s_wc[BINSCAN_NW];
     __shared__ unsigned short s_list[BINSCAN_LIST];  // tile groups whose window overlaps the block's cells
     __shared__ int s_part[BINSCAN_NW][33];
+    __shared__ int4 s_desc[BINSCAN_DESC];
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
     if (blockIdx.x * 32 >= a.n_sc) {
         // one extra block (species with an ordered absorbed list only): exclusive prefix of the per-tile
@@ -299,6 +301,59 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
     const int chunk = (n_virt + BINSCAN_NW - 1) / BINSCAN_NW;
     const int v_beg = min(wp * chunk, n_virt), v_end = min(v_beg + chunk, n_virt);
     constexpr int B = 8;  // tiles in flight per warp: the loads of a batch are independent
+    if (listed && n_virt <= BINSCAN_DESC) {
+        // usual case: the descriptors (lo, w, off) of the listed tiles are fetched once, coalesced, into
+        // shared memory; both passes then read them with one broadcast LDS.128 and no index arithmetic
+        for (int v = tid; v < n_virt; v += BINSCAN_NW * 32) {
+            const int t = (int)s_list[v / PIC1D_GROUP] * PIC1D_GROUP + v % PIC1D_GROUP;
+            s_desc[v] = t < n_tiles ? make_int4(a.tile_lo[t], a.tile_w[t], a.tile_off[t], 0) : make_int4(0, 0, 0, 0);
+        }
+        __syncthreads();
+        int sum = 0;
+        for (int v0 = v_beg; v0 < v_end; v0 += B) {
+            int c[B];
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                c[b] = 0;
+                if (v0 + b < v_end) {
+                    const int4 d = s_desc[v0 + b];
+                    const unsigned r = (unsigned)(k - d.x);
+                    if (r < (unsigned)d.y) c[b] = __ldcg(a.pool + d.z + r);
+                }
+            }
+#pragma unroll
+            for (int b = 0; b < B; ++b) sum += c[b];
+        }
+        s_part[wp][lane] = sum;
+        __syncthreads();
+        int run = 0, total = 0;
+#pragma unroll 8
+        for (int q = 0; q < BINSCAN_NW; ++q) {
+            const int v = s_part[q][lane];
+            if (q < wp) run += v;
+            total += v;
+        }
+        for (int v0 = v_beg; v0 < v_end; v0 += B) {
+            int* p[B];
+            int c[B];
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                p[b] = nullptr;
+                c[b] = 0;
+                if (v0 + b < v_end) {
+                    const int4 d = s_desc[v0 + b];
+                    const unsigned r = (unsigned)(k - d.x);
+                    if (r < (unsigned)d.y) p[b] = a.pool + d.z + r;
+                }
+            }
+#pragma unroll
+            for (int b = 0; b < B; ++b) if (p[b]) c[b] = __ldcg(p[b]);
+#pragma unroll
+            for (int b = 0; b < B; ++b) if (p[b]) { __stcg(p[b], run); run += c[b]; }
+        }
+        if (wp == 0 && k < a.n_sc) a.hist[k] = total;
+        return;
+    }
     int sum = 0;
     for (int v0 = v_beg; v0 < v_end; v0 += B) {
         int c[B];
