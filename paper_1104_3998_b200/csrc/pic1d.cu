@@ -122,7 +122,7 @@ size_t layout(pic1d* h, char* base) {
     h->T = cap_max >= 2048ll * 592 ? 2048 : 1024;
     const int rr = c.sort_inv_ratio < 1.0 ? (int)std::llround(1.0 / c.sort_inv_ratio) : 1;
     const int ppc_est = (int)std::max<int64_t>(1, cap_max / c.n_cells);
-    h->G = std::min(2048, std::max(rr, pow2_floor(std::max(1, 8192 / ppc_est))));
+    h->G = std::min(2048, std::max(rr, pow2_floor(std::max(1, 65536 / ppc_est))));
     h->n_dep_blocks = (c.n_cells + h->G - 1) / h->G;
     size_t off = 0;
     h->st = carve<DevState>(base, off, 1);

@@ -37,6 +37,47 @@ __device__ __forceinline__ long long warp_sum_ll(long long v) {
     return v;
 }
 
+struct DepAcc {  // a warp's register partial sums for its current cell
+    int jc, accn;
+    long long accF;
+};
+
+__device__ __forceinline__ void dep_flush(DepAcc& A, ull* s_acc, int c0, int lane) {
+    if (A.jc >= 0) {
+        const long long Fs = warp_sum_ll(A.accF);
+        const int n = __reduce_add_sync(0xffffffffu, A.accn);
+        if (lane == 0) {
+            atomicAdd(&s_acc[A.jc - c0], (ull)((long long)n * DEP_ONE - Fs));
+            atomicAdd(&s_acc[A.jc + 1 - c0], (ull)Fs);
+        }
+    }
+    A.accF = 0; A.accn = 0;
+}
+
+// one row of 32 slots (one particle per lane)
+__device__ __forceinline__ void dep_row(bool valid, float xv, DepAcc& A, ull* s_acc, int c0, int lane) {
+    const int j = (int)xv;
+    const long long F = __float2ll_rz(__fmul_rn(__fsub_rn(xv, (float)j), 0x1p40f));
+    const int j0 = __shfl_sync(0xffffffffu, j, 0);
+    if (__all_sync(0xffffffffu, valid && j == j0)) {
+        if (j0 != A.jc) { dep_flush(A, s_acc, c0, lane); A.jc = j0; }
+        A.accF += F; ++A.accn;
+    } else {  // the row straddles cells: one warp reduction per distinct cell
+        unsigned rem = __ballot_sync(0xffffffffu, valid);
+        while (rem) {
+            const int jj = __shfl_sync(0xffffffffu, j, __ffs(rem) - 1);
+            const bool in = valid && j == jj;
+            const unsigned grp = __ballot_sync(0xffffffffu, in);
+            const long long Fs = warp_sum_ll(in ? F : 0ll);
+            if (lane == 0) {
+                atomicAdd(&s_acc[jj - c0], (ull)((long long)__popc(grp) * DEP_ONE - Fs));
+                atomicAdd(&s_acc[jj + 1 - c0], (ull)Fs);
+            }
+            rem &= ~grp;
+        }
+    }
+}
+
 __global__ void __launch_bounds__(PIC1D_NT) k_deposit(DepositArgs a) {
     extern __shared__ ull s_acc[];  // G + 1 nodes
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
@@ -46,60 +87,47 @@ __global__ void __launch_bounds__(PIC1D_NT) k_deposit(DepositArgs a) {
     const int p0 = a.offsets[k0], p1 = a.offsets[k1];
     for (int i = tid; i <= a.G; i += PIC1D_NT) s_acc[i] = 0ull;
     __syncthreads();
-    const int rows_w = ((p1 - p0 + 31) / 32 + PIC1D_NWARP - 1) / PIC1D_NWARP;
-    const int beg = min(p0 + wp * rows_w * 32, p1), end = min(beg + rows_w * 32, p1);
-    int jc = -1, accn = 0;
-    long long accF = 0;
-    for (int i0 = beg; i0 < end; i0 += 32 * DEP_U) {
-        float xv[DEP_U];
-#pragma unroll
-        for (int u = 0; u < DEP_U; ++u) {
-            const int i = i0 + u * 32 + lane;
-            xv[u] = i < end ? __ldcs(a.x + i) : -1.0f;
+    // [p0, p1) = head [p0, a0) + 128-slot chunks [a0, a1) + tail [a1, p1); chunks are read as float4
+    const int a0 = min(p1, (p0 + 127) & ~127), a1 = max(a0, p1 & ~127);
+    DepAcc A;
+    A.jc = -1; A.accn = 0; A.accF = 0;
+    if (wp == 0) {  // head and tail, row by row
+        for (int i0 = p0; i0 < a0; i0 += 32) {
+            const int i = i0 + lane;
+            dep_row(i < a0, i < a0 ? __ldcs(a.x + i) : 0.0f, A, s_acc, c0, lane);
         }
+        for (int i0 = a1; i0 < p1; i0 += 32) {
+            const int i = i0 + lane;
+            dep_row(i < p1, i < p1 ? __ldcs(a.x + i) : 0.0f, A, s_acc, c0, lane);
+        }
+    }
+    const int ch_w = ((a1 - a0) / 128 + PIC1D_NWARP - 1) / PIC1D_NWARP;  // chunks per warp
+    const int cb = min(a0 + wp * ch_w * 128, a1), ce = min(cb + ch_w * 128, a1);
+    for (int i0 = cb; i0 < ce; i0 += 128 * DEP_U) {
+        float4 q[DEP_U];
+#pragma unroll
+        for (int u = 0; u < DEP_U; ++u)
+            if (i0 + u * 128 < ce) q[u] = __ldcs(reinterpret_cast<const float4*>(a.x + i0 + u * 128) + lane);
 #pragma unroll
         for (int u = 0; u < DEP_U; ++u) {
-            const bool valid = xv[u] >= 0.0f;
-            const int j = (int)xv[u];
-            const long long F = __float2ll_rz(__fmul_rn(__fsub_rn(xv[u], (float)j), 0x1p40f));
-            const int j0 = __shfl_sync(0xffffffffu, j, 0);
-            if (__all_sync(0xffffffffu, valid && j == j0)) {
-                if (j0 != jc) {
-                    if (jc >= 0) {
-                        const long long Fs = warp_sum_ll(accF);
-                        const int n = __reduce_add_sync(0xffffffffu, accn);
-                        if (lane == 0) {
-                            atomicAdd(&s_acc[jc - c0], (ull)((long long)n * DEP_ONE - Fs));
-                            atomicAdd(&s_acc[jc + 1 - c0], (ull)Fs);
-                        }
-                    }
-                    jc = j0; accF = 0; accn = 0;
-                }
-                accF += F; ++accn;
-            } else {  // the row straddles cells: one warp reduction per distinct cell
-                unsigned rem = __ballot_sync(0xffffffffu, valid);
-                while (rem) {
-                    const int jj = __shfl_sync(0xffffffffu, j, __ffs(rem) - 1);
-                    const bool in = valid && j == jj;
-                    const unsigned grp = __ballot_sync(0xffffffffu, in);
-                    const long long Fs = warp_sum_ll(in ? F : 0ll);
-                    if (lane == 0) {
-                        atomicAdd(&s_acc[jj - c0], (ull)((long long)__popc(grp) * DEP_ONE - Fs));
-                        atomicAdd(&s_acc[jj + 1 - c0], (ull)Fs);
-                    }
-                    rem &= ~grp;
-                }
+            if (i0 + u * 128 >= ce) break;  // warp-uniform
+            const int jx = (int)q[u].x, jy = (int)q[u].y, jz = (int)q[u].z, jw = (int)q[u].w;
+            const int j0 = __shfl_sync(0xffffffffu, jx, 0);
+            if (__all_sync(0xffffffffu, (jx == j0) & (jy == j0) & (jz == j0) & (jw == j0))) {
+                if (j0 != A.jc) { dep_flush(A, s_acc, c0, lane); A.jc = j0; }
+                const float fj = (float)j0;
+                A.accF += __float2ll_rz(__fmul_rn(__fsub_rn(q[u].x, fj), 0x1p40f)) +
+                          __float2ll_rz(__fmul_rn(__fsub_rn(q[u].y, fj), 0x1p40f)) +
+                          __float2ll_rz(__fmul_rn(__fsub_rn(q[u].z, fj), 0x1p40f)) +
+                          __float2ll_rz(__fmul_rn(__fsub_rn(q[u].w, fj), 0x1p40f));
+                A.accn += 4;
+            } else {  // the chunk straddles cells
+                dep_row(true, q[u].x, A, s_acc, c0, lane); dep_row(true, q[u].y, A, s_acc, c0, lane);
+                dep_row(true, q[u].z, A, s_acc, c0, lane); dep_row(true, q[u].w, A, s_acc, c0, lane);
             }
         }
     }
-    if (jc >= 0) {
-        const long long Fs = warp_sum_ll(accF);
-        const int n = __reduce_add_sync(0xffffffffu, accn);
-        if (lane == 0) {
-            atomicAdd(&s_acc[jc - c0], (ull)((long long)n * DEP_ONE - Fs));
-            atomicAdd(&s_acc[jc + 1 - c0], (ull)Fs);
-        }
-    }
+    dep_flush(A, s_acc, c0, lane);
     __syncthreads();
     for (int i = tid; i < a.G; i += PIC1D_NT) a.part[(size_t)blockIdx.x * a.G + i] = (double)s_acc[i] * 0x1p-40;
     if (tid == 0) a.side[blockIdx.x] = (double)s_acc[c1 - c0] * 0x1p-40;
