@@ -79,7 +79,12 @@ CASES = {
     "cfg2_ratio16": dict(cfg_id=2, n_cells=256, ppc=64, sort_ratio=16.0),
     "cfg1_small": dict(cfg_id=1, ppc=40),
     "cfg4_scaled": dict(cfg_id=4, n_cells=512, ppc=300),
+    "cfg2_courant": dict(cfg_id=2, n_cells=256, ppc=150, courant=True),   # Eq. 5 holds for both species
+    "cfg3_courant": dict(cfg_id=3, n_cells=512, ppc=260, courant=True),
 }
+# ions faster than a warp tile's 32-bin pool row: overflow rows, cursors in global memory
+FAST_IONS = {"fast_ions": (dict(cfg_id=2, n_cells=256, ppc=64), 40.0),
+             "fast_ions_wide": (dict(cfg_id=2, n_cells=1024, ppc=20), 300.0)}
 LONG = dict(CASES, cfg2_long=dict(cfg_id=2, n_cells=128, ppc=500))
 
 
@@ -97,6 +102,24 @@ def test_load_then_single_steps_from_identical_state(name):
         # step 1 starts from a bit-identical state; later steps inherit <= 1e-6 velocity differences
         # of collided / emitted particles (libm vs CUDA logf, sinf, cosf), so x is compared by tolerance
         compare_state(o, g, p, exact_x=(n == 0))
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("name", list(FAST_IONS))
+def test_ions_violating_eq5_take_the_wide_window_path(name):
+    kw, vth_i = FAST_IONS[name]
+    p = W.make_params(**kw)
+    p["vth"] = [p["vth"][0], vth_i]
+    o, g, p = _mk(p)
+    from oracle import oracle as O
+    from paper_1104_3998_b200 import pic1d as G
+    compare_state(o, g, p, check_keys=False)
+    for n in range(3):
+        g.set_E32(o.debug_get(O.E32))
+        assert o.step(1) == 0
+        g.step(1)
+        compare_state(o, g, p, exact_x=(n == 0))
+    assert int(g.debug_get(G.DBG_TILE_W, 1).max()) > 32
     o.close(); g.close()
 
 
