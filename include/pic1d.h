@@ -39,6 +39,10 @@ extern "C" {
 /* flags */
 #define PIC1D_FLAG_CAPTURE 1u /* keep per-slot pre-sort keys and MCC event masks for pic1d_debug_get */
 #define PIC1D_FLAG_VERIFY_ORDER 2u /* re-check every in-tile rank of the scatter with match.any (slow) */
+#define PIC1D_FLAG_EQ5_ELECTRONS 4u /* hint: the electrons obey Eq. 5 (L162: they move less than about one sort
+                                       cell per step), so they take the barrier-free warp-tile sort like the
+                                       ions.  Only a performance hint: both sort families are correct for any
+                                       displacement. */
 
 typedef struct pic1d pic1d_t; /* opaque */
 

@@ -147,7 +147,8 @@ size_t layout(pic1d* h, char* base) {
         p.cur = 0;
         for (int b = 0; b < 2; ++b)
             for (int k = 0; k < 4; ++k) p.buf[b][k] = carve<float>(base, off, p.capacity);
-        p.warp_tiles = s != 0;  // ions; electrons may move many cells per step (configs 2-4)
+        // ions always; electrons only on the caller's word: they may move many cells per step (configs 2-4)
+        p.warp_tiles = s != 0 || (c.flags & PIC1D_FLAG_EQ5_ELECTRONS) != 0;
         p.T = p.warp_tiles ? PIC1D_TW : h->T;
         p.n_tiles_max = p.capacity / p.T;
         p.n_groups_max = (p.n_tiles_max + PIC1D_GROUP - 1) / PIC1D_GROUP;

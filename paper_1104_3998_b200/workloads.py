@@ -68,6 +68,10 @@ def make_params(cfg_id, n_cells=None, ppc=None, sort_ratio=1.0, courant=False, s
              n_per_species=n_per_species, sort_ratio=float(sort_ratio),
              sort_inv_ratio=1.0 / float(sort_ratio), seed=int(c["seed"]), flags=int(flags),
              courant=bool(courant))
+    # performance hint for the library (PIC1D_FLAG_EQ5_ELECTRONS = 4): electron thermal displacement below
+    # one cell per step -- configs 0, 1 and the Courant-respecting twins
+    if cfg_id in (0, 1) or courant:
+        p["flags"] |= 4
     if cfg_id == 1:
         wpdt = 0.1
         p.update(n_species=1, background_rho=float(ppc_), V0_norm=0.0, omega_dt=0.0,

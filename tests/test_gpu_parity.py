@@ -19,7 +19,8 @@ def _mk(p):
     from oracle import oracle as O
     from paper_1104_3998_b200 import pic1d as G
     p = dict(p)
-    p["flags"] = G.FLAG_CAPTURE | G.FLAG_VERIFY_ORDER
+    hint = 0 if p.pop("no_hint", False) else (p["flags"] & G.FLAG_EQ5_ELECTRONS)
+    p["flags"] = G.FLAG_CAPTURE | G.FLAG_VERIFY_ORDER | hint
     parts = W.make_particles(p)
     o, g = O.Oracle(p), G.Pic1D(p)
     load(o, parts)
@@ -86,6 +87,22 @@ CASES = {
 FAST_IONS = {"fast_ions": (dict(cfg_id=2, n_cells=256, ppc=64), 40.0),
              "fast_ions_wide": (dict(cfg_id=2, n_cells=1024, ppc=20), 300.0)}
 LONG = dict(CASES, cfg2_long=dict(cfg_id=2, n_cells=128, ppc=500))
+
+
+def test_electron_hint_only_changes_the_kernel_family():
+    """configs 0 / 1 with the Eq. 5 hint cleared: narrow electron windows through the block-tile kernels"""
+    from oracle import oracle as O
+    for kw in (dict(cfg_id=0), dict(cfg_id=1, ppc=40), dict(cfg_id=2, n_cells=256, ppc=150, courant=True)):
+        p = W.make_params(**kw)
+        p["no_hint"] = True
+        o, g, p = _mk(p)
+        compare_state(o, g, p, check_keys=False)
+        for n in range(3):
+            g.set_E32(o.debug_get(O.E32))
+            assert o.step(1) == 0
+            g.step(1)
+            compare_state(o, g, p, exact_x=(n == 0))
+        o.close(); g.close()
 
 
 @pytest.mark.parametrize("name", list(CASES))
