@@ -122,7 +122,9 @@ size_t layout(pic1d* h, char* base) {
     h->T = cap_max >= 2048ll * 592 ? 2048 : 1024;
     const int rr = c.sort_inv_ratio < 1.0 ? (int)std::llround(1.0 / c.sort_inv_ratio) : 1;
     const int ppc_est = (int)std::max<int64_t>(1, cap_max / c.n_cells);
-    h->G = std::min(2048, std::max(rr, pow2_floor(std::max(1, 65536 / ppc_est))));
+    // cells per deposit block: ~32-64 k particles per block, but at least ~300 blocks when the grid allows
+    const int g_work = pow2_floor(std::max(1, 65536 / ppc_est)), g_par = pow2_floor(std::max(1, c.n_cells / 296));
+    h->G = std::min(2048, std::max(rr, std::min(g_work, g_par)));
     h->n_dep_blocks = (c.n_cells + h->G - 1) / h->G;
     size_t off = 0;
     h->st = carve<DevState>(base, off, 1);
@@ -311,7 +313,7 @@ void enqueue_grid(pic1d* h, unsigned n_time) {
         DepositArgs d;
         d.x = p.buf[p.cur][0]; d.offsets = p.offsets; d.part = p.part; d.side = p.side;
         d.Nc = c.n_cells; d.n_sc = h->n_sc; d.G = h->G; d.inv_r = h->inv_r;
-        k_deposit<<<h->n_dep_blocks, PIC1D_NT, (h->G + 1) * sizeof(ull), h->stream>>>(d);
+        k_deposit<<<h->n_dep_blocks, PIC1D_NT, (h->G + 1) * (sizeof(ull) + 3 * sizeof(unsigned)), h->stream>>>(d);
         mark(h, "deposit", s);
         cb.part[s] = p.part; cb.side[s] = p.side; cb.rho_s[s] = p.rho_s; cb.sign[s] = c.sp[s].charge_sign;
     }

@@ -54,15 +54,32 @@ __device__ __forceinline__ void dep_flush(DepAcc& A, ull* s_acc, int c0, int lan
     A.accF = 0; A.accn = 0;
 }
 
-// one row of 32 slots (one particle per lane)
-__device__ __forceinline__ void dep_row(bool valid, float xv, DepAcc& A, ull* s_acc, int c0, int lane) {
+// one row of 32 slots (one particle per lane).  A row that straddles cells (every row when a sort cell
+// holds several grid cells, r > 1) adds its two weights per lane as three 14-bit limbs with native 32-bit
+// shared reductions (conflicting red.shared is not serialised on sm_100a); `limbs` is off when the block
+// holds so many particles that a limb counter could overflow (2^18 additions), then the row is split by
+// cell value with one warp reduction per distinct cell.
+#define DEP_LIMB_MAX 200000
+__device__ __forceinline__ void dep_limbs(unsigned* s_l, int node, int np1, long long v) {
+    atomicAdd(&s_l[node], (unsigned)(v & 0x3fff));
+    atomicAdd(&s_l[np1 + node], (unsigned)((v >> 14) & 0x3fff));
+    atomicAdd(&s_l[2 * np1 + node], (unsigned)(v >> 28));
+}
+
+__device__ __forceinline__ void dep_row(bool valid, float xv, DepAcc& A, ull* s_acc, unsigned* s_l, int np1,
+                                        bool limbs, int c0, int lane) {
     const int j = (int)xv;
     const long long F = __float2ll_rz(__fmul_rn(__fsub_rn(xv, (float)j), 0x1p40f));
     const int j0 = __shfl_sync(0xffffffffu, j, 0);
     if (__all_sync(0xffffffffu, valid && j == j0)) {
         if (j0 != A.jc) { dep_flush(A, s_acc, c0, lane); A.jc = j0; }
         A.accF += F; ++A.accn;
-    } else {  // the row straddles cells: one warp reduction per distinct cell
+    } else if (limbs) {
+        if (valid) {
+            dep_limbs(s_l, j - c0, np1, DEP_ONE - F);
+            dep_limbs(s_l, j + 1 - c0, np1, F);
+        }
+    } else {  // one warp reduction per distinct cell
         unsigned rem = __ballot_sync(0xffffffffu, valid);
         while (rem) {
             const int jj = __shfl_sync(0xffffffffu, j, __ffs(rem) - 1);
@@ -79,13 +96,16 @@ __device__ __forceinline__ void dep_row(bool valid, float xv, DepAcc& A, ull* s_
 }
 
 __global__ void __launch_bounds__(PIC1D_NT) k_deposit(DepositArgs a) {
-    extern __shared__ ull s_acc[];  // G + 1 nodes
+    extern __shared__ ull s_acc[];  // G + 1 nodes, then 3 x (G + 1) 32-bit limb counters
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
     const int c0 = blockIdx.x * a.G, c1 = min(c0 + a.G, a.Nc);
     const int k0 = (int)__fmul_rn((float)c0, a.inv_r);
     const int k1 = c1 >= a.Nc ? a.n_sc : (int)__fmul_rn((float)c1, a.inv_r);
     const int p0 = a.offsets[k0], p1 = a.offsets[k1];
-    for (int i = tid; i <= a.G; i += PIC1D_NT) s_acc[i] = 0ull;
+    const int np1 = a.G + 1;
+    unsigned* s_l = reinterpret_cast<unsigned*>(s_acc + np1);
+    const bool limbs = p1 - p0 <= DEP_LIMB_MAX;  // block-uniform
+    for (int i = tid; i <= a.G; i += PIC1D_NT) { s_acc[i] = 0ull; s_l[i] = 0u; s_l[np1 + i] = 0u; s_l[2 * np1 + i] = 0u; }
     __syncthreads();
     // [p0, p1) = head [p0, a0) + 128-slot chunks [a0, a1) + tail [a1, p1); chunks are read as float4
     const int a0 = min(p1, (p0 + 127) & ~127), a1 = max(a0, p1 & ~127);
@@ -94,11 +114,11 @@ __global__ void __launch_bounds__(PIC1D_NT) k_deposit(DepositArgs a) {
     if (wp == 0) {  // head and tail, row by row
         for (int i0 = p0; i0 < a0; i0 += 32) {
             const int i = i0 + lane;
-            dep_row(i < a0, i < a0 ? __ldcs(a.x + i) : 0.0f, A, s_acc, c0, lane);
+            dep_row(i < a0, i < a0 ? __ldcs(a.x + i) : 0.0f, A, s_acc, s_l, np1, limbs, c0, lane);
         }
         for (int i0 = a1; i0 < p1; i0 += 32) {
             const int i = i0 + lane;
-            dep_row(i < p1, i < p1 ? __ldcs(a.x + i) : 0.0f, A, s_acc, c0, lane);
+            dep_row(i < p1, i < p1 ? __ldcs(a.x + i) : 0.0f, A, s_acc, s_l, np1, limbs, c0, lane);
         }
     }
     const int ch_w = ((a1 - a0) / 128 + PIC1D_NWARP - 1) / PIC1D_NWARP;  // chunks per warp
@@ -122,15 +142,18 @@ __global__ void __launch_bounds__(PIC1D_NT) k_deposit(DepositArgs a) {
                           __float2ll_rz(__fmul_rn(__fsub_rn(q[u].w, fj), 0x1p40f));
                 A.accn += 4;
             } else {  // the chunk straddles cells
-                dep_row(true, q[u].x, A, s_acc, c0, lane); dep_row(true, q[u].y, A, s_acc, c0, lane);
-                dep_row(true, q[u].z, A, s_acc, c0, lane); dep_row(true, q[u].w, A, s_acc, c0, lane);
+                dep_row(true, q[u].x, A, s_acc, s_l, np1, limbs, c0, lane); dep_row(true, q[u].y, A, s_acc, s_l, np1, limbs, c0, lane);
+                dep_row(true, q[u].z, A, s_acc, s_l, np1, limbs, c0, lane); dep_row(true, q[u].w, A, s_acc, s_l, np1, limbs, c0, lane);
             }
         }
     }
     dep_flush(A, s_acc, c0, lane);
     __syncthreads();
-    for (int i = tid; i < a.G; i += PIC1D_NT) a.part[(size_t)blockIdx.x * a.G + i] = (double)s_acc[i] * 0x1p-40;
-    if (tid == 0) a.side[blockIdx.x] = (double)s_acc[c1 - c0] * 0x1p-40;
+    auto node = [&](int i) {
+        return (double)(s_acc[i] + (ull)s_l[i] + ((ull)s_l[np1 + i] << 14) + ((ull)s_l[2 * np1 + i] << 28)) * 0x1p-40;
+    };
+    for (int i = tid; i < a.G; i += PIC1D_NT) a.part[(size_t)blockIdx.x * a.G + i] = node(i);
+    if (tid == 0) a.side[blockIdx.x] = node(c1 - c0);
 }
 
 // Follow-up kernel (L138): node j of species s = block part + the left neighbour's right-edge node;
