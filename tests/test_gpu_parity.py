@@ -38,6 +38,11 @@ def _vel_err(gv, ov):
 def compare_state(o, g, p, check_keys=True, exact_x=True):
     from oracle import oracle as O
     from paper_1104_3998_b200 import pic1d as G
+    vmax = 1.0
+    for s in range(p["n_species"]):
+        v2 = sum(o.debug_get(w, s).astype(np.float64) ** 2 for w in (O.VX, O.VY, O.VZ))
+        if v2.size:
+            vmax = max(vmax, float(np.sqrt(v2.max())))
     for s in range(p["n_species"]):
         mo, mg = o.moments(s), g.moments(s)
         for k in ("count", "n_sorted", "absorbed_left", "absorbed_right", "injected", "n_candidates",
@@ -51,7 +56,10 @@ def compare_state(o, g, p, check_keys=True, exact_x=True):
         if exact_x:
             assert np.array_equal(ox, gx), (s, np.nonzero(ox != gx)[0][:10])
         else:
-            assert np.max(np.abs(ox.astype(np.float64) - gx) / np.maximum(np.abs(ox), 1.0)) <= TOL_V
+            # not an identical state any more: x = x_old + vx inherits the <= 1e-6 |v| velocity difference of
+            # particles that collided in an earlier step, and an ion born in an ionisation inherits its parent
+            # electron's x -- so the bound uses the largest speed of any species
+            assert np.max(np.abs(ox.astype(np.float64) - gx) / np.maximum(np.abs(ox), vmax)) <= TOL_V
         ev = _vel_err([g.debug_get(w, s) for w in (G.DBG_VX, G.DBG_VY, G.DBG_VZ)],
                       [o.debug_get(w, s) for w in (O.VX, O.VY, O.VZ)])
         assert ev <= TOL_V, (s, ev)
@@ -301,4 +309,56 @@ def test_config4_full_size_in_bench_configuration():
     ro, po, Eo = o.get_rho_phi_E()
     rg, pg, Eg = g.get_rho_phi_E()
     assert rel_linf(rg, ro) <= TOL_RHO and rel_linf(pg, po) <= TOL_FIELD and rel_linf(Eg, Eo) <= TOL_FIELD
+    o.close(); g.close()
+
+
+def test_birth_capacity_overflow_matches_oracle():
+    """hot electrons ionise until the arrays are full: the same births are kept (lowest parent slots first),
+    the same number dropped, and both sides raise the sticky capacity error"""
+    from oracle import oracle as O
+    from paper_1104_3998_b200 import pic1d as G
+    p = W.make_params(4, n_cells=256, ppc=300, capacity_factor=1.0)
+    p["vth"] = [p["vth"][0] * 6.0, p["vth"][1]]
+    o, g, p = _mk(p)
+    rc_o = 0
+    for n in range(40):
+        g.set_E32(o.debug_get(O.E32))
+        rc_o = o.step(1)
+        g.step(1)
+        compare_state(o, g, p, exact_x=(n == 0))
+        if rc_o != 0:
+            break
+    assert rc_o == G.ERR_CAPACITY, "the case must reach the overflow (got %d after %d steps)" % (rc_o, n + 1)
+    assert g.moments(0)["dropped"] > 0 and g.moments(0)["sticky"] == G.ERR_CAPACITY
+    o.close(); g.close()
+
+
+def test_nonfinite_field_is_absorbed_and_flagged():
+    """a NaN in the gathered field: the particles of that cell get a NaN position, are absorbed (counted at
+    the right wall) and both sides raise the sticky non-finite error"""
+    from oracle import oracle as O
+    from paper_1104_3998_b200 import pic1d as G
+    o, g, p = _mk(W.make_params(2, n_cells=128, ppc=50, mcc=False, gamma=0.0))
+    e32 = o.debug_get(O.E32).copy()
+    e32[40] = np.nan
+    o.set_E32(e32); g.set_E32(e32)
+    rc_o = o.step(1)
+    g.step(1)
+    compare_state(o, g, p)
+    assert rc_o == G.ERR_NONFINITE and g.moments(0)["sticky"] == G.ERR_NONFINITE
+    assert g.moments(0)["absorbed_right"] >= 50
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("n_cells", [24576, 32768])
+def test_largest_grids(n_cells):
+    """24576 cells = the largest grid of the shared-memory field solve; 32768 takes the global-memory one"""
+    from oracle import oracle as O
+    o, g, p = _mk(W.make_params(2, n_cells=n_cells, ppc=6))
+    compare_state(o, g, p, check_keys=False)
+    for n in range(2):
+        g.set_E32(o.debug_get(O.E32))
+        assert o.step(1) == 0
+        g.step(1)
+        compare_state(o, g, p, exact_x=(n == 0))
     o.close(); g.close()
