@@ -362,3 +362,26 @@ def test_largest_grids(n_cells):
         g.step(1)
         compare_state(o, g, p, exact_x=(n == 0))
     o.close(); g.close()
+
+
+@pytest.mark.parametrize("kw,steps", [(dict(cfg_id=3), 15), (dict(cfg_id=3, courant=True), 15),
+                                      (dict(cfg_id=4, n_cells=2048, ppc=500), 40)])
+def test_gpu_run_is_bit_reproducible(kw, steps):
+    """two free runs from the same input give bit-identical particles and fields: no atomic, race or
+    scheduling order decides an index anywhere on the path (R18)"""
+    from paper_1104_3998_b200 import pic1d as G
+    p = W.make_params(**kw)
+    parts = W.make_particles(p)
+    res = []
+    for rep in range(2):
+        g = G.Pic1D(p)
+        load(g, parts)
+        g.step(steps)
+        out = [g.debug_get(w, s) for s in range(p["n_species"]) for w in (G.DBG_X, G.DBG_VX, G.DBG_VY, G.DBG_VZ)]
+        out += list(g.get_rho_phi_E())
+        out += [np.array([g.moments(s)[k] for k in ("count", "births", "injected", "n_candidates")])
+                for s in range(p["n_species"])]
+        res.append(out)
+        g.close()
+    for a, b in zip(*res):
+        assert np.array_equal(a, b)
