@@ -73,6 +73,15 @@ __device__ __forceinline__ unsigned lanemask_lt() {
     return m;
 }
 
+// shared-memory fetch-and-add issued by ONE lane that already carries a warp-aggregated value: plain
+// atom.shared, so that ptxas does not wrap it in its own (20-instruction) warp-aggregation sequence
+__device__ __forceinline__ int atom_shared_add(int* p, int v) {
+    int old;
+    const unsigned a = (unsigned)__cvta_generic_to_shared(p);
+    asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(a), "r"(v) : "memory");
+    return old;
+}
+
 __device__ __forceinline__ int warp_min(int v) {
 #pragma unroll
     for (int o = 16; o; o >>= 1) v = min(v, __shfl_xor_sync(0xffffffffu, v, o));

@@ -58,7 +58,7 @@ __device__ __forceinline__ ull desc_pack(uint32_t epoch, ull flag, int v) {
 __device__ __forceinline__ int warp_append(bool flag, int* counter) {
     const unsigned bal = __ballot_sync(0xffffffffu, flag);
     int base = 0;
-    if ((threadIdx.x & 31) == 0 && bal) base = atomicAdd(counter, __popc(bal));
+    if ((threadIdx.x & 31) == 0 && bal) base = atom_shared_add(counter, __popc(bal));
     base = __shfl_sync(0xffffffffu, base, 0);
     return base + __popc(bal & lanemask_lt());
 }
@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
                 if (lane >= o) inc += t;
             }
             int base = 0;
-            if (lane == 31 && inc) base = atomicAdd(&s_n[0], inc);
+            if (lane == 31 && inc) base = atom_shared_add(&s_n[0], inc);
             base = __shfl_sync(0xffffffffu, base, 31) + inc - cnt;
             if (STAGE) {  // most slots are candidates: predicated stores
 #pragma unroll
