@@ -317,7 +317,8 @@ def main():
                        "l2": "inputs larger than L2 (%.2f GB of particle state per GPU)" % (n_mean * 16 / 1e9),
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "capture_masks": False,
-                       "sort": "electrons: block tiles of 2048 slots (staged scatter); ions: warp tiles of 256 slots"},
+                       "sort": ("electrons and ions: warp tiles of 256 slots" if p["flags"] & 4 else
+                                "electrons: block tiles of 2048 slots (staged scatter); ions: warp tiles of 256 slots")},
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": args.e2e_steps, "note": "load_particles(host) + step(1) + get_rho_phi_E(host) per step"},
