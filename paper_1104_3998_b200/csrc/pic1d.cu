@@ -362,7 +362,9 @@ void enqueue_mcc(pic1d* h) {
         m.null_any = thr > 0;
         m.null_le = (uint32_t)(thr - 1);
         const int grid = std::min(p.n_mcc_tiles, h->num_sms * 4);
-        const bool stage = c.sp[s].P0 > 0.25;
+        // STAGE (velocities streamed into shared memory during the null test) is compiled but not selected:
+        // measured 0.624 ms staged (3 blocks/SM) vs 0.610 ms unstaged (4 blocks/SM) for config-4 electrons
+        const bool stage = false;
         if (m.kind == 1) {
             if (stage) k_mcc<1, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE_STAGE * sizeof(float), h->stream>>>(m);
             else k_mcc<1, false><<<grid, PIC1D_NT, MCC_TILE * sizeof(float), h->stream>>>(m);
