@@ -207,7 +207,10 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
                 __threadfence();
             }
             int excl = 0;
-            int j = tile - 1;  // this probe looks at tiles j, j-1, ..., j-31
+            // a tile without ionisations needs no prefix of its own: it leaves its aggregate (0) for the
+            // tiles behind it to walk through and does not wait for anybody
+            const bool need = nb > 0 || tile == n_act - 1;
+            int j = need ? tile - 1 : -1;  // this probe looks at tiles j, j-1, ..., j-31
             while (j >= 0) {
                 const int idx = j - lane;
                 const ull d = idx >= 0 ? desc[idx] : desc_pack(epoch, DESC_PREFIX, 0);  // before tile 0: prefix 0
@@ -226,7 +229,7 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
                 }                                 // else: somebody nearer than any prefix is not there yet: probe again
             }
             if (lane == 0) {
-                if (tile > 0) {
+                if (tile > 0 && need) {
                     desc[tile] = desc_pack(epoch, DESC_PREFIX, excl + nb);
                     __threadfence();
                 }
