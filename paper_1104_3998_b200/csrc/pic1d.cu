@@ -3,7 +3,8 @@
 // One stream-ordered kernel sequence per step, no host round trip (contrast PAPER.md L144):
 //   k_step_begin
 //   per species (ions first, so their wall hits can emit secondaries into the electron source):
-//       k_push_count -> k_bin_scan -> k_offsets_scan -> k_push_scatter [-> k_see_emit]
+//       k_push_count[_w] -> k_bin_scan -> k_offsets_scan -> k_push_scatter[_w] [-> k_see_emit]
+//       (_w: barrier-free warp-tile kernels for species that obey Eq. 5, pic1d_sort_warp.cuh)
 //   k_deposit per species -> k_rho_combine -> k_field -> k_mcc per species
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -fmad=false (see ../build.py).
 #include <cmath>

@@ -8,10 +8,12 @@
 //                           shared memory; the tile's window [lo, hi] of counts goes to a pool
 //   scan    k_bin_scan      per sort cell k: exclusive prefix over tiles of count[t][k] (in place),
 //                           total -> hist[k]
-//           k_offsets_scan  exclusive scan of hist -> offsets[N_sc + 1]; prefix of absorbed counts
+//                           (+ one extra block: prefix of the per-tile absorbed counts)
+//           k_offsets_scan  exclusive scan of hist -> offsets[N_sc + 1]
 //   pass 2  k_push_scatter  read x, vx, vy, vz (16 B); identical push; stable rank inside the tile
-//                           (warp match + shared counters, warps in order); write the four arrays to
-//                           offsets[k] + prefix[t][k] + rank (16 B)
+//                           (warp-private shared counters, warps in order); write the four arrays to
+//                           offsets[k] + prefix[t][k] + rank (16 B), through a tile-sorted shared-memory
+//                           staging buffer when the tile spreads over many cells
 //
 // A tile is T consecutive source slots.  Because the source is sorted by last step's cell, a tile's
 // keys fall in a narrow window when particles move about one cell per step (Eq. 5); nothing
