@@ -405,3 +405,49 @@ def test_gpu_run_is_bit_reproducible(kw, steps):
         g.close()
     for a, b in zip(*res):
         assert np.array_equal(a, b)
+
+
+def test_config3_full_size_100_step_moments_within_1pct():
+    """config 3 at its full size, free-running for 100 steps: time-averaged densities and potential and the
+    energy moments within 1 % of the oracle (north_star's long-run bar; trajectories diverge chaotically)"""
+    from oracle import oracle as O
+    from paper_1104_3998_b200 import pic1d as G
+    p = W.make_params(3)
+    parts = W.make_particles(p)
+    o, g = O.Oracle(p), G.Pic1D(p)
+    load(o, parts); load(g, parts)
+    acc = [0.0] * 6
+    for n in range(100):
+        assert o.step(1) == 0
+        g.step(1)
+        if n % 5 == 4:
+            mo, mg = [o.moments(s) for s in range(2)], [g.moments(s) for s in range(2)]
+            acc[0] = acc[0] + mo[0]["density"]; acc[1] = acc[1] + mg[0]["density"]
+            acc[2] = acc[2] + mo[1]["density"]; acc[3] = acc[3] + mg[1]["density"]
+            acc[4] = acc[4] + o.get_rho_phi_E()[1]; acc[5] = acc[5] + g.get_rho_phi_E()[1]
+            for s in range(2):
+                assert abs(mg[s]["sum_v2"] / mg[s]["count"] / (mo[s]["sum_v2"] / mo[s]["count"]) - 1) <= 0.01
+                assert abs(mg[s]["sum_v4"] / mg[s]["count"] / (mo[s]["sum_v4"] / mo[s]["count"]) - 1) <= 0.02
+                assert abs(mg[s]["count"] / mo[s]["count"] - 1) <= 0.01
+    assert rel_l2(acc[1], acc[0]) <= 0.01 and rel_l2(acc[3], acc[2]) <= 0.01 and rel_l2(acc[5], acc[4]) <= 0.01
+    assert g.moments(0)["sticky"] == 0
+    o.close(); g.close()
+
+
+def test_config4_200_steps_bookkeeping():
+    """the bench workload over config 4's own 200 steps (GPU only): no sticky error, and every species'
+    count balances: loaded - absorbed + births + injected (- nothing dropped)"""
+    from paper_1104_3998_b200 import pic1d as G
+    p = W.make_params(4)
+    g = G.Pic1D(p)
+    load(g, W.make_particles(p))
+    for chunk in range(4):
+        g.step(50)
+        for s in range(2):
+            m = g.moments(s)
+            assert m["sticky"] == 0 and m["dropped"] == 0
+            assert m["count"] == p["n_per_species"] - m["absorbed_left"] - m["absorbed_right"] + m["births"] + m["injected"]
+        r, ph, E = g.get_rho_phi_E()
+        assert np.all(np.isfinite(r)) and np.all(np.isfinite(ph)) and np.all(np.isfinite(E))
+        assert abs(r.sum() - (g.moments(1)["n_sorted"] - g.moments(0)["n_sorted"])) <= 1e-6 * p["n_per_species"]
+    g.close()
