@@ -351,7 +351,12 @@ void enqueue_mcc(pic1d* h) {
             m.ix = pi.buf[pi.cur][0]; m.ivx = pi.buf[pi.cur][1]; m.ivy = pi.buf[pi.cur][2]; m.ivz = pi.buf[pi.cur][3];
             m.cap_i = pi.capacity;
         }
-        m.st = h->st; m.desc = p.desc; m.mask = p.mask;
+        m.st = h->st; m.mask = p.mask;
+        // ionisation records: per-tile counts + (slot, speed) lists in the electrons' INACTIVE buffer, which
+        // is scratch until the next step's scatter writes into it
+        m.rec_nb = reinterpret_cast<int*>(p.desc);
+        m.rec_rel = reinterpret_cast<int*>(pe.buf[pe.cur ^ 1][2]);
+        m.rec_gp = pe.buf[pe.cur ^ 1][3];
         m.s = s; m.kind = c.sp[s].mcc_kind; m.n_species = c.n_species;
         m.step = h->step; m.k0 = (uint32_t)c.seed; m.k1 = (uint32_t)(c.seed >> 32);
         m.P0 = (float)c.sp[s].P0; m.inv_g_cap = (float)c.sp[s].inv_g_cap; m.c_eV = (float)c.sp[s].c_eV;
@@ -368,7 +373,11 @@ void enqueue_mcc(pic1d* h) {
         const bool stage = false;
         if (m.kind == 1) {
             if (stage) k_mcc<1, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE_STAGE * sizeof(float), h->stream>>>(m);
-            else k_mcc<1, false><<<grid, PIC1D_NT, MCC_TILE * sizeof(float), h->stream>>>(m);
+            else k_mcc<1, false><<<grid, PIC1D_NT, 0, h->stream>>>(m);
+            mark(h, "mcc", s);
+            k_mcc_births<<<h->num_sms, PIC1D_NT, 0, h->stream>>>(m);
+            mark(h, "mcc_births", s);
+            continue;
         } else {
             if (stage) k_mcc<2, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE_STAGE * sizeof(float), h->stream>>>(m);
             else k_mcc<2, false><<<grid, PIC1D_NT, 0, h->stream>>>(m);

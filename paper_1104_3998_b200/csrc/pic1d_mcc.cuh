@@ -9,13 +9,12 @@
 //   phase B  one thread per CANDIDATE: load v, Philox (u_type, ...), process selection (no
 //            transcendental); real collisions are compacted into a second list
 //   phase C  one thread per REAL COLLISION: kinematics (sqrt, sincos, log), velocity written back
-//   phase D  one thread per IONISATION: the new electron / ion pair
+//   k_mcc_births  one thread per IONISATION: the new electron / ion pair
 // Ionisation products go to the tails of the electron / ion arrays in ascending parent-slot order
 // (the paper allocates them with a shared counter inside the parent's sort cell, L203; here the tail
 // is sorted into place by the next step's fine sort).  The order inside a tile comes from a bit mask
-// over its slots, the order across tiles from a decoupled look-back over per-tile ionisation counts
-// (tiles are handed out by a ticket, so every predecessor of a tile is already running) -- no
-// atomic decides any index.
+// over its slots, the order across tiles from the prefix of the per-tile ionisation counts that
+// k_mcc_births forms -- no atomic decides any index.
 #pragma once
 #include "pic1d_device.cuh"
 
@@ -27,7 +26,9 @@ struct MccArgs {
     float *ex, *evx, *evy, *evz;  // electron buffer (birth tail)
     float *ix, *ivx, *ivy, *ivz;  // ion buffer (birth tail), may be null
     DevState* st;
-    ull* desc;       // look-back descriptors, one per tile
+    int* rec_nb;     // [tile] ionisations of the tile (electron set)
+    int* rec_rel;    // [tile * MCC_TILE + r] parent slot - tile base of the tile's r-th ionisation, slot order
+    float* rec_gp;   // [tile * MCC_TILE + r] speed shared by its two electrons
     uint8_t* mask;   // optional event mask per sorted slot
     int s, kind, n_species, cap_e, cap_i;
     uint32_t step, k0, k1;
@@ -48,12 +49,6 @@ __device__ __forceinline__ float bm_r(float u) {
     return sqrtf(__fmul_rn(-2.0f, logf(__fsub_rn(1.0f, u))));
 }
 
-#define DESC_AGG 1ull
-#define DESC_PREFIX 2ull
-__device__ __forceinline__ ull desc_pack(uint32_t epoch, ull flag, int v) {
-    return ((ull)epoch << 32) | (flag << 30) | (ull)(unsigned)v;
-}
-
 // append `flag`-ged items of a warp to a shared list; returns this lane's index (valid if flag)
 __device__ __forceinline__ int warp_append(bool flag, int* counter) {
     const unsigned bal = __ballot_sync(0xffffffffu, flag);
@@ -69,8 +64,8 @@ __device__ __forceinline__ int warp_append(bool flag, int* counter) {
 template <int KIND, bool STAGE>
 __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
     constexpr int TILE = STAGE ? MCC_TILE_STAGE : MCC_TILE;
-    extern __shared__ float s_v[];  // STAGE: [3][TILE] velocities; else (KIND 1): [TILE] speeds of ionising slots
-    __shared__ int s_tile, s_excl;
+    extern __shared__ float s_v[];  // STAGE: [3][TILE] velocities
+    __shared__ int s_tile;
     __shared__ int s_n[3];                          // candidates, real collisions, ionisations
     __shared__ unsigned short s_cand[TILE];     // slot - tile base
     __shared__ unsigned short s_coll[TILE];     // (slot - tile base) | event << 12
@@ -80,12 +75,9 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
     DevSpecies& sp = st->sp[a.s];
     const int n_sorted = sp.n_sorted;
     const int n_act = (n_sorted + TILE - 1) / TILE;
-    const uint32_t epoch = a.step + 1u;
     const uint32_t str_null = STREAM_NULL + (uint32_t)a.s, str_coll = STREAM_COLL + (uint32_t)a.s;
     int c_cand = 0, c_e0 = 0, c_e1 = 0, c_e2 = 0, c_e3 = 0, c_over = 0;
     float* s_vx = s_v; float* s_vy = s_v + TILE; float* s_vz = s_v + 2 * TILE;
-    unsigned short* s_ion_rel = s_cand;  // ionising slots in slot order (the candidate list is dead by then)
-    float* s_gp = s_v;                   // [slot - tile base] speed shared by the two electrons (its vx is dead by then)
     while (true) {
         if (tid == 0) { s_tile = atomicAdd(&sp.ticket, 1); s_n[0] = 0; s_n[1] = 0; s_n[2] = 0; }
         if (tid < TILE / 32) s_ionbits[tid] = 0u;
@@ -196,64 +188,9 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
         }
         c_e0 += c_pack & 0xff; c_e1 += (c_pack >> 8) & 0xff; c_e2 += (c_pack >> 16) & 0xff; c_e3 += c_pack >> 24;
         __syncthreads();
-        // ---- ordered births: publish this tile's ionisation count, then the exclusive prefix over earlier
-        // tiles by a warp-wide decoupled look-back (32 predecessors per probe), while the other warps
-        // already run phase C ----------------------------------------------------------------------
+        // ---- ionisations of the tile: count now, records in phase C, the pairs themselves in k_mcc_births
         const int nb = s_n[2];
-        if (KIND == 1 && tid < 32) {
-            volatile ull* desc = a.desc;
-            if (lane == 0) {
-                desc[tile] = desc_pack(epoch, tile == 0 ? DESC_PREFIX : DESC_AGG, nb);
-                __threadfence();
-            }
-            int excl = 0;
-            // a tile without ionisations needs no prefix of its own: it leaves its aggregate (0) for the
-            // tiles behind it to walk through and does not wait for anybody
-            const bool need = nb > 0 || tile == n_act - 1;
-            int j = need ? tile - 1 : -1;  // this probe looks at tiles j, j-1, ..., j-31
-            while (j >= 0) {
-                const int idx = j - lane;
-                const ull d = idx >= 0 ? desc[idx] : desc_pack(epoch, DESC_PREFIX, 0);  // before tile 0: prefix 0
-                const bool ready = (uint32_t)(d >> 32) == epoch;
-                const bool is_p = ready && ((d >> 30) & 3ull) == DESC_PREFIX;
-                const unsigned nr = __ballot_sync(0xffffffffu, !ready), pm = __ballot_sync(0xffffffffu, is_p);
-                const int first_p = pm ? __ffs(pm) - 1 : 32, first_nr = nr ? __ffs(nr) - 1 : 32;
-                const int v = (int)(d & 0x3fffffffull);
-                if (first_p < first_nr) {         // a prefix, and everything nearer than it is published
-                    excl += __reduce_add_sync(0xffffffffu, lane <= first_p ? v : 0);
-                    break;
-                }
-                if (first_nr == 32) {             // 32 aggregates: take them all, look further back
-                    excl += __reduce_add_sync(0xffffffffu, v);
-                    j -= 32;
-                }                                 // else: somebody nearer than any prefix is not there yet: probe again
-            }
-            if (lane == 0) {
-                if (tile > 0 && need) {
-                    desc[tile] = desc_pack(epoch, DESC_PREFIX, excl + nb);
-                    __threadfence();
-                }
-                s_excl = excl;
-                if (tile == n_act - 1) {  // last tile: close the step's birth bookkeeping
-                    const int total = excl + nb;
-                    const int ne = st->sp[0].n_sorted;
-                    int room = a.cap_e - ne;
-                    if (a.n_species > 1) room = min(room, a.cap_i - st->sp[1].n_sorted);
-                    const int kept = min(total, max(room, 0));
-                    st->sp[0].n_live = ne + kept;
-                    st->sp[0].births += (ull)kept;
-                    if (a.n_species > 1) {
-                        st->sp[1].n_live = st->sp[1].n_sorted + kept;
-                        st->sp[1].births += (ull)kept;
-                    }
-                    if (total > kept) {
-                        st->sp[0].dropped += (ull)(total - kept);
-                        if (a.n_species > 1) st->sp[1].dropped += (ull)(total - kept);
-                        atomicOr(&st->err, ERRBIT_CAPACITY);
-                    }
-                }
-            }
-        }
+        if (KIND == 1 && tid == 0) a.rec_nb[tile] = nb;
         // ---- phase C: kinematics, one thread per real collision -------------------------------------
         const int n_coll = s_n[1];
         for (int j = tid; j < n_coll; j += PIC1D_NT) {
@@ -281,8 +218,8 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
                     // rank among the tile's ionisations in slot order
                     int r = __popc(s_ionbits[rel >> 5] & ((1u << (rel & 31)) - 1u));
                     for (int q = 0; q < (rel >> 5); ++q) r += __popc(s_ionbits[q]);
-                    s_ion_rel[r] = (unsigned short)rel;
-                    s_gp[rel] = gp;
+                    a.rec_rel[tbase + r] = rel;
+                    a.rec_gp[tbase + r] = gp;
                 }
                 a.vx[i] = __fmul_rn(gp, n[0]); a.vy[i] = __fmul_rn(gp, n[1]); a.vz[i] = __fmul_rn(gp, n[2]);
             } else {
@@ -293,39 +230,6 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
                 a.vx[i] = __fmul_rn(a.gvt, __fmul_rn(r12, cosf(ph12)));
                 a.vy[i] = __fmul_rn(a.gvt, __fmul_rn(r12, sinf(ph12)));
                 a.vz[i] = __fmul_rn(a.gvt, __fmul_rn(r3, cosf(ph3)));
-            }
-        }
-        if (KIND != 1) { __syncthreads(); continue; }
-        __syncthreads();
-        // ---- phase D: one thread per ionisation: the new electron / ion pair -------------------------
-        if (nb > 0) {
-            const int ne = st->sp[0].n_sorted, ni = a.n_species > 1 ? st->sp[1].n_sorted : 0;
-            int room = a.cap_e - ne;
-            if (a.n_species > 1) room = min(room, a.cap_i - ni);
-            for (int r = tid; r < nb; r += PIC1D_NT) {
-                const int b = s_excl + r;  // birth index of the step, ascending parent slot
-                if (b >= room) continue;
-                const uint32_t i = (uint32_t)(tbase + s_ion_rel[r]);
-                uint32_t b0[4], b1[4], b2[4];
-                philox4x32_10(i, a.step, str_coll, 0u, a.k0, a.k1, b0);
-                philox4x32_10(i, a.step, str_coll, 1u, a.k0, a.k1, b1);
-                philox4x32_10(i, a.step, str_coll, 2u, a.k0, a.k1, b2);
-                const float xp = a.x[i];
-                float n2[3];
-                iso_dir(u01(b0[3]), u01(b1[0]), n2);
-                const float gp = s_gp[s_ion_rel[r]];
-                const int de = ne + b;
-                a.ex[de] = xp;
-                a.evx[de] = __fmul_rn(gp, n2[0]); a.evy[de] = __fmul_rn(gp, n2[1]); a.evz[de] = __fmul_rn(gp, n2[2]);
-                if (a.n_species > 1) {
-                    const float r12 = bm_r(u01(b1[1])), ph12 = __fmul_rn(6.2831855f, u01(b1[2]));
-                    const float r3 = bm_r(u01(b1[3])), ph3 = __fmul_rn(6.2831855f, u01(b2[0]));
-                    const int di = ni + b;
-                    a.ix[di] = xp;
-                    a.ivx[di] = __fmul_rn(a.gvt, __fmul_rn(r12, cosf(ph12)));
-                    a.ivy[di] = __fmul_rn(a.gvt, __fmul_rn(r12, sinf(ph12)));
-                    a.ivz[di] = __fmul_rn(a.gvt, __fmul_rn(r3, cosf(ph3)));
-                }
             }
         }
         __syncthreads();
@@ -340,6 +244,106 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
 #pragma unroll
             for (int q = 0; q < 4; ++q) if (vals[1 + q]) atomicAdd(&sp.n_events[q], (ull)vals[1 + q]);
             if (vals[5]) atomicAdd(&sp.over_cap, (ull)vals[5]);
+        }
+    }
+}
+
+// ---- the ionisation pairs (L203), in ascending parent-slot order ---------------------------------------
+// k_mcc left, per tile, the number of ionisations and their (parent slot, electron speed) records in slot
+// order.  Birth index = (ionisations of all earlier tiles) + (rank inside the tile): every block takes a
+// contiguous chunk of tiles, sums the counts of the tiles before its chunk itself (a few 10^4 integers
+// from L2, read coalesced) and scans its own chunk -- nobody waits for anybody.  A decoupled look-back
+// inside k_mcc did the same job first; it cost 15-20 % of that kernel, because the tiles in flight wait
+// for each other's counts at a barrier (profiles/r1_notes.md).
+__global__ void __launch_bounds__(PIC1D_NT) k_mcc_births(MccArgs a) {
+    __shared__ int s_w[PIC1D_NWARP + 1];
+    __shared__ int s_pre[PIC1D_NT], s_cnt[PIC1D_NT];
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    DevState* st = a.st;
+    const int n_sorted = st->sp[a.s].n_sorted;
+    const int n_act = (n_sorted + MCC_TILE - 1) / MCC_TILE;
+    const int chunk = (n_act + gridDim.x - 1) / gridDim.x;
+    const int t0 = min(blockIdx.x * chunk, n_act), t1 = min(t0 + chunk, n_act);
+    if (t0 >= t1) return;
+    auto block_sum = [&](int v) -> int {
+        v = __reduce_add_sync(0xffffffffu, v);
+        __syncthreads();
+        if (lane == 0) s_w[wp] = v;
+        __syncthreads();
+        int t = 0;
+#pragma unroll
+        for (int q = 0; q < PIC1D_NWARP; ++q) t += s_w[q];
+        return t;
+    };
+    int part = 0;
+    for (int t = tid; t < t0; t += PIC1D_NT) part += a.rec_nb[t];
+    int base = block_sum(part);  // ionisations of the tiles before this block's chunk
+    const int ne = st->sp[0].n_sorted, ni = a.n_species > 1 ? st->sp[1].n_sorted : 0;
+    int room = a.cap_e - ne;
+    if (a.n_species > 1) room = min(room, a.cap_i - ni);
+    const uint32_t str_coll = STREAM_COLL + (uint32_t)a.s;
+    for (int c0 = t0; c0 < t1; c0 += PIC1D_NT) {
+        const int nt = min(PIC1D_NT, t1 - c0);
+        const int v = tid < nt ? a.rec_nb[c0 + tid] : 0;
+        int inc = v;  // exclusive scan of the piece's counts
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        __syncthreads();
+        if (lane == 31) s_w[wp] = inc;
+        __syncthreads();
+        int before = 0, tot = 0;
+#pragma unroll
+        for (int q = 0; q < PIC1D_NWARP; ++q) { const int u = s_w[q]; if (q < wp) before += u; tot += u; }
+        s_pre[tid] = base + before + inc - v;
+        s_cnt[tid] = v;
+        __syncthreads();
+        for (int q = wp; q < nt; q += PIC1D_NWARP) {  // one warp per tile
+            const int nbq = s_cnt[q], tbase = (c0 + q) * MCC_TILE;
+            for (int r = lane; r < nbq; r += 32) {
+                const int b = s_pre[q] + r;  // birth index of the step, ascending parent slot
+                if (b >= room) continue;
+                const uint32_t i = (uint32_t)(tbase + a.rec_rel[tbase + r]);
+                uint32_t b0[4], b1[4], b2[4];
+                philox4x32_10(i, a.step, str_coll, 0u, a.k0, a.k1, b0);
+                philox4x32_10(i, a.step, str_coll, 1u, a.k0, a.k1, b1);
+                philox4x32_10(i, a.step, str_coll, 2u, a.k0, a.k1, b2);
+                const float xp = a.x[i];
+                float n2[3];
+                iso_dir(u01(b0[3]), u01(b1[0]), n2);
+                const float gp = a.rec_gp[tbase + r];
+                const int de = ne + b;
+                a.ex[de] = xp;
+                a.evx[de] = __fmul_rn(gp, n2[0]); a.evy[de] = __fmul_rn(gp, n2[1]); a.evz[de] = __fmul_rn(gp, n2[2]);
+                if (a.n_species > 1) {
+                    const float r12 = bm_r(u01(b1[1])), ph12 = __fmul_rn(6.2831855f, u01(b1[2]));
+                    const float r3 = bm_r(u01(b1[3])), ph3 = __fmul_rn(6.2831855f, u01(b2[0]));
+                    const int di = ni + b;
+                    a.ix[di] = xp;
+                    a.ivx[di] = __fmul_rn(a.gvt, __fmul_rn(r12, cosf(ph12)));
+                    a.ivy[di] = __fmul_rn(a.gvt, __fmul_rn(r12, sinf(ph12)));
+                    a.ivz[di] = __fmul_rn(a.gvt, __fmul_rn(r3, cosf(ph3)));
+                }
+            }
+        }
+        base += tot;
+        __syncthreads();
+    }
+    if (t1 == n_act && tid == 0) {  // the block with the last tile closes the step's birth bookkeeping
+        const int total = base;
+        const int kept = min(total, max(room, 0));
+        st->sp[0].n_live = ne + kept;
+        st->sp[0].births += (ull)kept;
+        if (a.n_species > 1) {
+            st->sp[1].n_live = ni + kept;
+            st->sp[1].births += (ull)kept;
+        }
+        if (total > kept) {
+            st->sp[0].dropped += (ull)(total - kept);
+            if (a.n_species > 1) st->sp[1].dropped += (ull)(total - kept);
+            atomicOr(&st->err, ERRBIT_CAPACITY);
         }
     }
 }
