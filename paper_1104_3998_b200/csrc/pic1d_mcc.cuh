@@ -91,7 +91,9 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
         unsigned bits = 0;  // bit 4 q + c: slot c of the thread's quad q is a candidate
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
-            const int rel0 = (q * PIC1D_NT + tid) * 4, i0 = tbase + rel0;
+            // a thread owns 4 NQ CONSECUTIVE slots, so the candidate list below comes out in slot order and
+            // the per-candidate phase reads neighbouring velocities
+            const int rel0 = (tid * NQ + q) * 4, i0 = tbase + rel0;
             if (tile_full || i0 < n_sorted) {
                 float4 A, B, C;
                 if (STAGE) {  // buffers have capacity slots (a multiple of 4096): the vector never leaves them
@@ -128,12 +130,12 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
             if (STAGE) {  // most slots are candidates: predicated stores
 #pragma unroll
                 for (int b = 0; b < 4 * NQ; ++b)
-                    if ((bits >> b) & 1u) s_cand[base++] = (unsigned short)(((b >> 2) * PIC1D_NT + tid) * 4 + (b & 3));
+                    if ((bits >> b) & 1u) s_cand[base++] = (unsigned short)(tid * (4 * NQ) + b);
             } else {      // few are: walk the set bits
                 while (bits) {
                     const int b = __ffs(bits) - 1;
                     bits &= bits - 1;
-                    s_cand[base++] = (unsigned short)(((b >> 2) * PIC1D_NT + tid) * 4 + (b & 3));
+                    s_cand[base++] = (unsigned short)(tid * (4 * NQ) + b);
                 }
             }
         }
