@@ -451,3 +451,35 @@ def test_config4_200_steps_bookkeeping():
         assert np.all(np.isfinite(r)) and np.all(np.isfinite(ph)) and np.all(np.isfinite(E))
         assert abs(r.sum() - (g.moments(1)["n_sorted"] - g.moments(0)["n_sorted"])) <= 1e-6 * p["n_per_species"]
     g.close()
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("PIC1D_SLOW"), reason="~20 min of single-threaded oracle time: set PIC1D_SLOW=1")
+def test_config4_full_size_200_step_moments_within_1pct():
+    """BASELINE.json config 4 exactly as specified (1.31e8 particles, 200 steps), free-running on both sides:
+    time-averaged densities and potential and the energy moments within 1 % (north_star).  Opt-in because the
+    oracle needs ~5 s per step; the outcome of the last run is recorded in profiles/r1_configs.md."""
+    from oracle import oracle as O
+    from paper_1104_3998_b200 import pic1d as G
+    p = W.make_params(4)
+    parts = W.make_particles(p)
+    o, g = O.Oracle(p), G.Pic1D(p)
+    load(o, parts); load(g, parts)
+    del parts
+    acc = [0.0] * 6
+    worst = [0.0, 0.0, 0.0]
+    for n in range(200):
+        assert o.step(1) == 0
+        g.step(1)
+        if n % 10 == 9:
+            mo, mg = [o.moments(s) for s in range(2)], [g.moments(s) for s in range(2)]
+            acc[0] = acc[0] + mo[0]["density"]; acc[1] = acc[1] + mg[0]["density"]
+            acc[2] = acc[2] + mo[1]["density"]; acc[3] = acc[3] + mg[1]["density"]
+            acc[4] = acc[4] + o.get_rho_phi_E()[1]; acc[5] = acc[5] + g.get_rho_phi_E()[1]
+            for s in range(2):
+                worst[0] = max(worst[0], abs(mg[s]["sum_v2"] / mg[s]["count"] / (mo[s]["sum_v2"] / mo[s]["count"]) - 1))
+                worst[1] = max(worst[1], abs(mg[s]["sum_v4"] / mg[s]["count"] / (mo[s]["sum_v4"] / mo[s]["count"]) - 1))
+                worst[2] = max(worst[2], abs(mg[s]["count"] / mo[s]["count"] - 1))
+    res = (rel_l2(acc[1], acc[0]), rel_l2(acc[3], acc[2]), rel_l2(acc[5], acc[4]))
+    print("config4 200 steps: rel L2 n_e %.3e n_i %.3e phi %.3e; worst <v2> %.3e <v4> %.3e count %.3e" % (res + tuple(worst)))
+    assert max(res) <= 0.01 and worst[0] <= 0.01 and worst[1] <= 0.02 and worst[2] <= 0.01
+    o.close(); g.close()
