@@ -21,17 +21,26 @@
  *   5 Poisson (Thomas) + E                 Eq. 1-2 (L113-117), L142-146
  *   6 modified null-collision Monte-Carlo collisions   L196-209, Eq. 6 (L200)
  *
- * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"):
- *   philox        : cuRAND host generator CURAND_RNG_PHILOX4_32_10 (independent code),
- *                   bijectivity on a sub-cube, uniformity
- *   push          : constant-field and linear-field closed forms (leapfrog)
- *   deposit       : sum(rho_s) == N_s exactly, single particle, brute-force hat sum
- *   field solve   : uniform / sinusoidal / Laplace closed forms, dense numpy solve
- *   whole loop    : cold plasma oscillation frequency (config 1), momentum conservation
- *   boundary      : bookkeeping, order, SEE binomial
- *   sort          : permutation, brute-force offsets, stability
- *   MCC           : null-collision statistics (Eq. 6), beam fractions, kinematic
+ * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"), per function:
+ *   philox4x32_10 : cuRAND host generator CURAND_RNG_PHILOX4_32_10 (independent code),
+ *                   bijectivity on two 2^16 sub-cubes of the counter space, uniformity
+ *   u01           : range / mean / chi^2 of U(r); Eq. 6 candidate rate
+ *   push (step 1) : constant-field and linear-field closed forms (leapfrog), linear gather
+ *   boundary, SEE : bookkeeping, ties at the walls, order, SEE binomial + Rayleigh moments;
+ *                   periodic wrap incl. the |v| > N_c / non-finite clamp (R21)
+ *   sort_species  : permutation, brute-force offsets, stability, numpy stable argsort
+ *   deposit       : sum(rho_s) == N_s exactly, single particle, brute-force hat sum, wrap
+ *   thomas_dirichlet, field_solve (the function the cycle runs; oracle_solve_field calls it):
+ *                   uniform / sinusoidal / Laplace / single-sheet closed forms incl. both
+ *                   wall nodes, Gauss's law over the gap, dense numpy solve; the uniform
+ *                   plasma through load -> sort -> deposit -> field_solve of the full Oracle
+ *   mcc           : null-collision statistics (Eq. 6); beam fractions against values built
+ *                   from the physical inputs (n_g, sigma_k(E), v(E), dt); kinematic
  *                   invariants (energy bookkeeping, isotropy, Maxwellian moments)
+ *   oracle_moments: numpy sums and numpy.histogram on the arrays debug_get returns;
+ *                   Maxwellian <v^2>, <v^4>
+ *   whole loop    : cold plasma oscillation frequency (config 1), momentum conservation
+ *   binary_collide (f3), reflect (f4), gapped sort (f2): see their own headers below
  *   long RF discharge physics (configs 2-4): parity unpinned beyond bookkeeping.
  */
 #include <math.h>
@@ -274,13 +283,14 @@ static void thomas_dirichlet(int n, const double* rhs, double* phi, double* cp) 
     for (int j = n - 2; j >= 1; --j) dp[j] = dp[j] - cp[j] * dp[j + 1];
 }
 
-/* ---- step 5: Poisson + E (Eq. 1-2) at time t_n = n_time * dt. */
-static void field_solve(orc_t* o, uint32_t n_time) {
+/* ---- step 5: Poisson + E (Eq. 1-2) for the wall potentials phi_0 = phi0 and
+ * phi_{N_c} = phiN (bounded; ignored for periodic runs). */
+static void field_solve(orc_t* o, double phi0, double phiN) {
     int Nc = o->cfg.n_cells;
     double *rho = o->rho, *phi = o->phi, *E = o->E;
     if (o->cfg.bc == 0) {
-        phi[0] = o->cfg.V0_norm * sin(o->cfg.omega_dt * (double)n_time);
-        phi[Nc] = 0.0;
+        phi[0] = phi0;
+        phi[Nc] = phiN;
         thomas_dirichlet(Nc, rho, phi, o->tmp);
         for (int j = 1; j < Nc; ++j) E[j] = (phi[j - 1] - phi[j + 1]) / 2.0;
         /* half-cell Gauss law with the RAW wall-node sums (R7) */
@@ -306,6 +316,11 @@ static void field_solve(orc_t* o, uint32_t n_time) {
         for (int j = 0; j < Nc; ++j) phi[j] -= pm;
     }
     for (int j = 0; j < o->nodes; ++j) o->E32[j] = (float)E[j];
+}
+
+/* wall potentials at time t_n = n_time * dt (R6): node 0 driven, node N_c grounded */
+static void field_solve_at(orc_t* o, uint32_t n_time) {
+    field_solve(o, o->cfg.V0_norm * sin(o->cfg.omega_dt * (double)n_time), 0.0);
 }
 
 /* isotropic unit vector from two uniforms (R14) */
@@ -528,7 +543,7 @@ static void step_once(orc_t* o) {
     /* 3. sort   4. deposit   5. field at t_{n+1}   6. MCC */
     for (int s = 0; s < c->n_species; ++s) sort_species(o, s);
     deposit(o);
-    field_solve(o, o->step + 1u);
+    field_solve_at(o, o->step + 1u);
     mcc(o);
     o->step += 1u;
 }
@@ -564,7 +579,7 @@ int oracle_load_particles(orc_t* o, int s, int64_t n, const float* x, const floa
             memset(pq->mask, 0, (size_t)o->cfg.sp[q].capacity);
         }
         deposit(o);
-        field_solve(o, 0u);
+        field_solve_at(o, 0u);
     }
     return 0;
 }
@@ -658,10 +673,11 @@ int oracle_n_sort_cells(orc_t* o) { return o ? o->n_sc : -1; }
 int oracle_n_nodes(orc_t* o) { return o ? o->nodes : -1; }
 uint32_t oracle_step_index(orc_t* o) { return o ? o->step : 0u; }
 
-/* Stand-alone pieces for the closed-form pins (tests call these on small arrays). */
+/* Stand-alone entry for the closed-form pins: runs field_solve() itself -- the function the cycle
+ * executes -- on a caller-supplied rho with the wall potentials given directly.  phi and E must
+ * hold nodes + 1 doubles (periodic: slot N_c is the wrap node). */
 int oracle_solve_field(int n_cells, int bc, const double* rho, double phi0, double phiN,
                        double* phi, double* E) {
-    /* same arithmetic as field_solve(), with the wall potentials given directly */
     orc_t o;
     memset(&o, 0, sizeof(o));
     o.cfg.n_cells = n_cells; o.cfg.bc = bc;
@@ -669,20 +685,7 @@ int oracle_solve_field(int n_cells, int bc, const double* rho, double phi0, doub
     o.rho = (double*)rho; o.phi = phi; o.E = E;
     o.tmp = calloc((size_t)n_cells + 2, 8);
     o.E32 = calloc((size_t)n_cells + 2, 4);
-    if (bc == 0) {
-        phi[0] = phi0; phi[n_cells] = phiN;
-        thomas_dirichlet(n_cells, rho, phi, o.tmp);
-        for (int j = 1; j < n_cells; ++j) E[j] = (phi[j - 1] - phi[j + 1]) / 2.0;
-        E[0] = (phi[0] - phi[1]) - rho[0];
-        E[n_cells] = (phi[n_cells - 1] - phi[n_cells]) + rho[n_cells];
-    } else {
-        /* periodic needs one more slot in phi for the wrap node */
-        double* ph = calloc((size_t)n_cells + 1, 8);
-        o.phi = ph;
-        field_solve(&o, 0u);
-        memcpy(phi, ph, (size_t)n_cells * 8);
-        free(ph);
-    }
+    field_solve(&o, phi0, phiN);
     free(o.tmp); free(o.E32);
     return 0;
 }

@@ -1,5 +1,7 @@
 """P3 / P4 / P11 -- oracle Poisson + E (Eq. 1-2; Thomas, L142) against closed forms
-and a dense numpy solve.  Wall-node E uses the half-cell Gauss law (R7)."""
+and a dense numpy solve.  Wall-node E uses the half-cell Gauss law (R7).
+O.solve_field() runs the oracle's field_solve() itself (the function the cycle executes), so a
+wrong sign or index in its wall-node terms fails the closed forms below."""
 import numpy as np
 import pytest
 
@@ -90,3 +92,66 @@ def test_rf_drive_no_charge_uniform_E():
         rho, phi, E = o.get_rho_phi_E()
         assert not rho.any()
         assert np.allclose(E, p["V0_norm"] * np.sin(p["omega_dt"] * n) / 16, rtol=1e-12)
+
+
+@pytest.mark.parametrize("Nc,f", [(8, 0.5), (64, 0.5), (33, 0.25)])
+def test_uniform_plasma_through_the_full_cycle(Nc, f):
+    """P3 through the full Oracle (load -> sort -> deposit -> field_solve): one ion per cell at the
+    same offset f gives rho_j = 1 at interior nodes and the raw wall sums 1 - f and f.  For f = 1/2
+    that is the uniform plasma with half-volume wall nodes: phi_j = j (N_c - j) / 2 and
+    E_j = j - N_c / 2 at EVERY node including the walls (Eq. 1-2; R7).  For
+    f != 1/2 the interior is the same parabola shifted by the wall-charge asymmetry; the wall
+    fields follow from Gauss's law over the whole gap: E_N - E_0 = total charge = N_c."""
+    p = params(2, n_cells=Nc, ppc=1, mcc=False, gamma=0.0)
+    p["V0_norm"] = 0.0
+    o = O.Oracle(p)
+    z = np.zeros(0, np.float32)
+    xi = (np.arange(Nc) + f).astype(np.float32)
+    load(o, [(z, z, z, z), (xi, 0 * xi, 0 * xi, 0 * xi)])
+    rho, phi, E = o.get_rho_phi_E()
+    want = np.ones(Nc + 1)
+    want[0], want[-1] = 1 - f, f
+    assert np.array_equal(rho, want)
+    j = np.arange(Nc + 1)
+    assert np.isclose(E[-1] - E[0], Nc, rtol=1e-12)                  # Gauss over the gap
+    assert np.allclose(np.diff(E)[1:-1], 1.0, rtol=1e-10)              # dE/dx = rho in the interior
+    if f == 0.5:
+        assert np.allclose(phi, j * (Nc - j) / 2, rtol=1e-12, atol=1e-12 * Nc * Nc)
+        assert np.allclose(E, j - Nc / 2, rtol=1e-11, atol=1e-11 * Nc)
+    else:
+        # interior Poisson residual and the half-cell wall law, written out from Eq. 1-2
+        assert np.allclose(phi[:-2] - 2 * phi[1:-1] + phi[2:], -rho[1:-1], atol=1e-10 * Nc)
+        assert np.isclose(E[0], (phi[0] - phi[1]) - (1 - f), rtol=1e-12, atol=1e-12)
+        assert np.isclose(E[-1], (phi[-2] - phi[-1]) + f, rtol=1e-12, atol=1e-12)
+        # a wall-sign error would break the symmetry E_j(f) + E_{N-j}(1-f) = 0
+    # mirror symmetry: reflecting the plasma (f -> 1 - f) reflects and negates E
+    o2 = O.Oracle(p)
+    xi2 = (np.arange(Nc) + (1 - f)).astype(np.float32)
+    load(o2, [(z, z, z, z), (xi2, 0 * xi2, 0 * xi2, 0 * xi2)])
+    _, phi2, E2 = o2.get_rho_phi_E()
+    assert np.allclose(E2, -E[::-1], rtol=1e-11, atol=1e-11 * Nc)
+    assert np.allclose(phi2, phi[::-1], rtol=1e-11, atol=1e-11 * Nc * Nc)
+
+
+def test_wall_field_signs_single_sheet():
+    """one positive charge sheet at node m between grounded walls (closed form of the discrete
+    Green's function): phi_j = j (N - m) / N for j <= m, m (N - j) / N beyond; E is piecewise
+    constant: -(N - m) / N left of the sheet and +m / N right of it, INCLUDING the wall nodes
+    (rho_0 = rho_N = 0 there).  Pins the sign convention E = -dphi/dx at both walls."""
+    N, m = 20, 7
+    rho = np.zeros(N + 1)
+    rho[m] = 1.0
+    phi, E = O.solve_field(N, 0, rho)
+    j = np.arange(N + 1)
+    assert np.allclose(phi, np.where(j <= m, j * (N - m) / N, m * (N - j) / N), atol=1e-13)
+    assert np.isclose(E[0], -(N - m) / N) and np.isclose(E[N], m / N)
+    assert np.allclose(E[1:m], -(N - m) / N) and np.allclose(E[m + 1:N], m / N)
+    # charge ON a wall node: the wall-node term of the half-cell law carries it (R7)
+    rho = np.zeros(N + 1)
+    rho[0] = 2.0
+    phi, E = O.solve_field(N, 0, rho)
+    assert not phi.any() and np.isclose(E[0], -2.0) and not E[1:].any()
+    rho = np.zeros(N + 1)
+    rho[N] = 3.0
+    phi, E = O.solve_field(N, 0, rho)
+    assert not phi.any() and np.isclose(E[N], 3.0) and not E[:N].any()

@@ -177,6 +177,71 @@ def test_secondary_emission_binomial_and_placement():
     assert abs(np.mean(vy)) < 4 * p["see_vth"] / np.sqrt(k)
 
 
+def test_periodic_clamp_faster_than_a_box_length_and_nan():
+    """DESIGN.md R21 (L41 says only "removed"/"inserted" for bounded runs; periodic comes from
+    BASELINE.json): ONE wrap is applied per step; a particle that is still outside [0, N_c)
+    afterwards (|v| > N_c, or a non-finite position) is put at x = 0, so every later array index
+    stays inside the grid."""
+    Nc = 16
+    o = O.Oracle(_one_species(Nc, 0.0, bc=1))
+    x0 = np.array([8.0, 8.0, 8.0, 8.0, 8.0, 15.5], np.float32)
+    v0 = np.array([20.0, 40.0, -40.0, -20.0, np.inf, 0.5], np.float32)
+    tag = np.arange(6, dtype=np.float32)
+    load(o, [(x0, v0, tag, tag)])
+    o.set_E32(np.zeros(Nc, np.float32))
+    o.step(1)
+    got = dict(zip(o.debug_get(O.VY).tolist(), o.debug_get(O.X).tolist()))
+    #   28 - 16 = 12 | 48 - 16 = 32 -> 0 | -32 + 16 = -16 -> 0 | -12 + 16 = 4 | inf -> 0 | 16 - 16 = 0
+    assert got == {0.0: 12.0, 1.0: 0.0, 2.0: 0.0, 3.0: 4.0, 4.0: 0.0, 5.0: 0.0}
+    assert o.moments(0)["count"] == 6 and o.moments(0)["absorbed_left"] == 0
+    # NaN field -> NaN position -> x = 0 (periodic runs never lose a particle)
+    o = O.Oracle(_one_species(Nc, 1.0, bc=1))
+    load(o, [(np.array([3.5], np.float32),) + (np.zeros(1, np.float32),) * 3])
+    e = np.zeros(Nc, np.float32)
+    e[3] = np.nan
+    o.set_E32(e)
+    o.step(1)
+    assert o.debug_get(O.X).tolist() == [0.0] and o.moments(0)["count"] == 1
+
+
+# ---- moments / EEDF (diagnostics of pic1d_moments) ---------------------------------------------
+def test_moments_and_eedf_against_numpy():
+    """oracle_moments() against numpy on the arrays debug_get returns: sums of v, |v|^2, |v|^4 over ALL
+    live slots (sorted part + birth tail) and the histogram of E = c_eV |v|^2 on [0, E_max)."""
+    p = params(2, n_cells=32, ppc=400)
+    o = O.Oracle(p)
+    from paper_1104_3998_b200 import workloads as W
+    p["vth"] = [3 * p["vth"][0], p["vth"][1]]     # 18 eV electrons: ionisation births within 3 steps
+    load(o, W.make_particles(p))
+    o.step(3)                                     # births in the tail, collided velocities
+    for s in range(2):
+        n_bins, E_max = 37, (60.0 if s == 0 else 0.2)
+        m = o.moments(s, n_bins=n_bins, E_max=E_max)
+        v = np.stack([o.debug_get(w, s) for w in (O.VX, O.VY, O.VZ)], 1).astype(np.float64)
+        assert m["count"] == v.shape[0] and m["count"] >= m["n_sorted"] > 0
+        if s == 0:
+            assert m["count"] > m["n_sorted"]     # the case has a birth tail
+        g2 = (v ** 2).sum(1)
+        for k, want in (("sum_vx", v[:, 0].sum()), ("sum_vy", v[:, 1].sum()), ("sum_vz", v[:, 2].sum())):
+            assert abs(m[k] - want) <= 1e-12 * np.abs(v).sum(), k
+        assert abs(m["sum_v2"] / g2.sum() - 1) < 1e-12 and abs(m["sum_v4"] / (g2 ** 2).sum() - 1) < 1e-12
+        En = p["species"][s]["c_eV"] * g2
+        h, _ = np.histogram(En[En < E_max], bins=n_bins, range=(0.0, E_max))
+        assert m["eedf"].sum() == (En < E_max).sum() > 0
+        # bin edges are floating-point: allow a particle sitting on an edge to fall either side
+        assert np.abs(np.cumsum(m["eedf"]) - np.cumsum(h)).max() <= 1
+        dens = m["density"]
+        assert dens.sum() == m["n_sorted"]        # density = rho_s of the last deposit (sorted part only)
+    # a Maxwellian's moments: <v^2> = 3 vth^2, <v^4> = 15 vth^4 (fresh load, nothing collided yet)
+    o = O.Oracle(p)
+    load(o, W.make_particles(p))
+    m = o.moments(1)
+    assert m["count"] == m["n_sorted"] == p["n_per_species"]
+    vt = p["vth"][1]
+    assert abs(m["sum_v2"] / m["count"] / (3 * vt ** 2) - 1) < 0.03
+    assert abs(m["sum_v4"] / m["count"] / (15 * vt ** 4) - 1) < 0.08
+
+
 # ---- P8 sort ---------------------------------------------------------------------------------
 @pytest.mark.parametrize("inv_ratio", [2.0, 1.0, 0.5, 0.0625])
 def test_sort_is_stable_permutation_with_bruteforce_offsets(inv_ratio):

@@ -53,8 +53,11 @@ def test_philox_counter_words_all_matter_and_bijective():
         seen.add(w)
     assert tuple(O.philox(4, 10, 20, 30, 40)) not in seen
     assert tuple(O.philox(3 + (1 << 32), 10, 20, 30, 40)) not in seen
-    outs = {tuple(O.philox(9, a, b, 0, 0)) for a in range(64) for b in range(64)}
-    assert len(outs) == 64 * 64
+    # bijective per key: no collision on a 2^16 sub-cube of the counter space
+    outs = {tuple(O.philox(9, a, b, 0, 0)) for a in range(256) for b in range(256)}
+    assert len(outs) == 1 << 16
+    outs = {tuple(O.philox(9, 5, 0, c, d)) for c in range(256) for d in range(256)}
+    assert len(outs) == 1 << 16
 
 
 def test_uniformity_chi2():
