@@ -159,6 +159,9 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fold", action="store_true",
+                    help="run the collisions as a pass of their own (k_mcc) instead of folded into the scatter")
+    ap.add_argument("--fold-all", action="store_true", help="fold the collisions of every species into its scatter")
     ap.add_argument("--profile", action="store_true",
                     help="timed region only (no per-kernel pass, e2e or CPU baseline): the command ncu wraps")
     args = ap.parse_args()
@@ -168,6 +171,10 @@ def main():
                       courant=args.courant)
     if args.impl == "reference":
         return reference_arm(args, p)
+    if args.no_fold:
+        p["flags"] |= 8   # PIC1D_FLAG_NO_FOLD
+    if args.fold_all:
+        p["flags"] |= 16  # PIC1D_FLAG_FOLD_ALL
 
     import torch
     import torch.distributed as dist

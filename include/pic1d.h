@@ -34,15 +34,22 @@ extern "C" {
 #define PIC1D_ERR_CUDA (-3)      /* a CUDA call failed; see pic1d_last_cuda_error */
 #define PIC1D_ERR_NONFINITE (-4) /* sticky: a NaN position was seen (treated as absorbed) */
 #define PIC1D_ERR_WORKSPACE (-5) /* workspace too small / sort bookkeeping pool exhausted (sticky) */
-#define PIC1D_ERR_ORDER (-6)     /* sticky: the rank self-check of PIC1D_FLAG_VERIFY_ORDER failed */
+#define PIC1D_ERR_ORDER (-6)     /* retired (never returned): the scatter ranks by construction now */
 
 /* flags */
 #define PIC1D_FLAG_CAPTURE 1u /* keep per-slot pre-sort keys and MCC event masks for pic1d_debug_get */
-#define PIC1D_FLAG_VERIFY_ORDER 2u /* re-check every in-tile rank of the scatter with match.any (slow) */
+#define PIC1D_FLAG_VERIFY_ORDER 2u /* retired, ignored: every in-tile rank of the scatter now comes from match.any
+                                      groups in slot order, so there is no hardware ordering left to verify */
 #define PIC1D_FLAG_EQ5_ELECTRONS 4u /* hint: the electrons obey Eq. 5 (L162: they move less than about one sort
                                        cell per step), so they take the barrier-free warp-tile sort like the
                                        ions.  Only a performance hint: both sort families are correct for any
                                        displacement. */
+
+/* Where the Monte-Carlo collisions of a species run (same results either way).  Default: folded into the
+ * scatter of its fine sort when its null-collision probability P0 <= 0.25 (sparse candidates), as a pass of
+ * its own after the field solve (k_mcc) otherwise. */
+#define PIC1D_FLAG_NO_FOLD 8u   /* never fold: every species gets the pass of its own */
+#define PIC1D_FLAG_FOLD_ALL 16u /* always fold */
 
 typedef struct pic1d pic1d_t; /* opaque */
 

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpic1d.so")
 SOURCES = ["pic1d.cu"]
-DEPS = ["pic1d.cu", "pic1d_device.cuh", "pic1d_sort.cuh", "pic1d_grid.cuh", "pic1d_mcc.cuh"]
+DEPS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh")))   # every source under csrc/
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false",
               "-std=c++17", "-shared", "-Xcompiler", "-fPIC"]
 

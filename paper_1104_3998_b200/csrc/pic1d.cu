@@ -15,10 +15,10 @@
 
 #include "../../include/pic1d.h"
 #include "pic1d_device.cuh"
+#include "pic1d_mcc.cuh"
 #include "pic1d_sort.cuh"
 #include "pic1d_sort_warp.cuh"
 #include "pic1d_grid.cuh"
-#include "pic1d_mcc.cuh"
 
 namespace {
 
@@ -33,8 +33,9 @@ struct SpeciesHost {
     int *hist, *offsets, *keys_dbg;
     uint8_t* mask;
     double *part, *side, *rho_s;
-    ull* desc;
     int n_mcc_tiles;
+    unsigned* null_bits;  // folded MCC: null-test bit per sorted slot of this step
+    int mcck;  // 0: the MCC of the species is a pass of its own (k_mcc) or absent; 1 / 2: folded into the scatter
 };
 
 struct TimeMark {
@@ -56,6 +57,10 @@ struct pic1d {
     float* E32;
     unsigned* abs_list;
     int abs_cap;
+    unsigned* ion_bits;  // ionisation records of the electron set (pic1d_mcc.cuh)
+    float* ion_gp;
+    int* ion_nb;
+    int n_ion_words;
     ull* eedf_dev;
     int eedf_cap;
     uint32_t step;
@@ -63,10 +68,10 @@ struct pic1d {
     bool ready;
     int64_t launches;
     cudaError_t last_err;
-    int grid_count[2], grid_scatter[2], WA;
+    int grid_count[2], grid_scatter[2][2], WA;
     size_t smem_sort, smem_count[2], smem_scatter[2];
     void (*k_count[2])(SortArgs);
-    void (*k_scatter[2])(SortArgs);
+    void (*k_scatter[2][2])(SortArgs);  // [species][0 plain | 1 the step's, with the MCC folded in]
     bool timing;
     std::vector<TimeMark> marks;
     std::vector<cudaEvent_t> ev_pool;
@@ -76,6 +81,7 @@ struct pic1d {
 namespace {
 
 const int MOM_BLOCKS = 1024;
+const double PIC1D_FOLD_P0_MAX = 0.25;
 const int EEDF_MAX_BINS = 65536;
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -180,8 +186,20 @@ size_t layout(pic1d* h, char* base) {
         p.part = carve<double>(base, off, (size_t)h->n_dep_blocks * h->G);
         p.side = carve<double>(base, off, h->n_dep_blocks);
         p.rho_s = carve<double>(base, off, h->nodes + 1);
-        p.n_mcc_tiles = (p.capacity + MCC_TILE_STAGE - 1) / MCC_TILE_STAGE;
-        p.desc = carve<ull>(base, off, p.n_mcc_tiles);
+        p.n_mcc_tiles = (p.capacity + MCC_TILE - 1) / MCC_TILE;
+        // fold the species' MCC into its scatter when its null-test candidates are sparse (the scatter's idle
+        // issue slots absorb them); a species most of whose particles are candidates keeps the compacting
+        // pass of its own (k_mcc) -- measured, DESIGN.md section 6.  The flags force either choice.
+        const bool sparse = c.sp[s].P0 <= PIC1D_FOLD_P0_MAX;
+        p.mcck = (c.flags & PIC1D_FLAG_NO_FOLD) ? 0 : (((c.flags & PIC1D_FLAG_FOLD_ALL) || sparse) ? c.sp[s].mcc_kind : 0);
+        p.null_bits = p.mcck ? carve<unsigned>(base, off, p.capacity / 32) : nullptr;
+    }
+    h->ion_bits = nullptr; h->ion_gp = nullptr; h->ion_nb = nullptr; h->n_ion_words = 0;
+    if (c.sp[0].mcc_kind == 1) {
+        h->n_ion_words = h->sp[0].capacity / 32;
+        h->ion_bits = carve<unsigned>(base, off, h->n_ion_words);
+        h->ion_gp = carve<float>(base, off, h->sp[0].capacity);
+        h->ion_nb = carve<int>(base, off, h->sp[0].n_mcc_tiles);
     }
     return align_up(off, 256);
 }
@@ -204,6 +222,25 @@ void mark(pic1d* h, const char* name, int species) {
     h->marks.push_back(TimeMark{name, species, e});
 }
 
+MccP mcc_params(pic1d* h, int s) {
+    const pic1d_config_t& c = h->cfg;
+    MccP m;
+    memset(&m, 0, sizeof(m));
+    m.st = h->st; m.mask = h->sp[s].mask; m.null_bits = h->sp[s].null_bits;
+    m.ion_bits = h->ion_bits; m.ion_gp = h->ion_gp; m.ion_nb = h->ion_nb;
+    m.s = s; m.kind = c.sp[s].mcc_kind;
+    m.k0 = (uint32_t)c.seed; m.k1 = (uint32_t)(c.seed >> 32);
+    m.inv_g_cap = (float)c.sp[s].inv_g_cap; m.c_eV = (float)c.sp[s].c_eV;
+    m.r_el = (float)c.r_el; m.r_exc = (float)c.r_exc; m.r_ion = (float)c.r_ion;
+    m.E_exc = (float)c.E_exc; m.E_ion = (float)c.E_ion;
+    m.two_mr = (float)(2.0 * c.mass_ratio); m.gvt = (float)c.gas_vth_ion;
+    // null test in integers: U(w) = (w >> 8) 2^-24 < P0  <=>  (w >> 8) < ceil(P0 2^24)  <=>  w <= null_le
+    const uint64_t thr = (uint64_t)std::ceil((double)(float)c.sp[s].P0 * 16777216.0) << 8;
+    m.null_any = thr > 0;
+    m.null_le = (uint32_t)(thr - 1);
+    return m;
+}
+
 SortArgs sort_args(pic1d* h, int s) {
     SpeciesHost& p = h->sp[s];
     SortArgs a;
@@ -218,7 +255,8 @@ SortArgs sort_args(pic1d* h, int s) {
     a.abs_cap = h->abs_cap;
     a.kappa = (float)h->cfg.sp[s].kappa;
     a.fNc = (float)h->cfg.n_cells; a.inv_r = h->inv_r; a.Nc = h->cfg.n_cells; a.n_sc = h->n_sc;
-    a.shift = 0; a.WA = h->WA; a.verify = (h->cfg.flags & PIC1D_FLAG_VERIFY_ORDER) ? 1 : 0;
+    a.shift = 0; a.WA = h->WA;
+    a.m = mcc_params(h, s);
     return a;
 }
 
@@ -229,16 +267,28 @@ sort_kernel_t count_kernel(int bc, int T) {
     return T == 2048 ? k_push_count<0, 2> : k_push_count<0, 1>;
 }
 
-// abs: the species records its absorbed slots (ions with secondary emission); stage: the species may
-// spread a tile over many bins (electrons), see k_push_scatter
-sort_kernel_t scatter_kernel(int bc, int T, bool abs, bool stage) {
-    if (bc == 1) {
-        if (stage) return T == 2048 ? k_push_scatter<1, 8, false, true> : k_push_scatter<1, 4, false, true>;
-        return T == 2048 ? k_push_scatter<1, 8, false, false> : k_push_scatter<1, 4, false, false>;
-    }
-    if (abs) return T == 2048 ? k_push_scatter<0, 8, true, false> : k_push_scatter<0, 4, true, false>;
-    if (stage) return T == 2048 ? k_push_scatter<0, 8, false, true> : k_push_scatter<0, 4, false, true>;
-    return T == 2048 ? k_push_scatter<0, 8, false, false> : k_push_scatter<0, 4, false, false>;
+// block tiles (species 0 only).  stage: the species may spread a tile over many bins (electrons), see
+// k_push_scatter; mcck: the electron collision set is folded in
+template <int BC, int MCCK>
+sort_kernel_t scatter_kernel_bm(int T, bool stage) {
+    if (stage) return T == 2048 ? k_push_scatter<BC, 8, true, MCCK> : k_push_scatter<BC, 4, true, MCCK>;
+    return T == 2048 ? k_push_scatter<BC, 8, false, MCCK> : k_push_scatter<BC, 4, false, MCCK>;
+}
+sort_kernel_t scatter_kernel(int bc, int T, bool stage, int mcck) {
+    if (bc == 1) return mcck == 1 ? scatter_kernel_bm<1, 1>(T, stage) : scatter_kernel_bm<1, 0>(T, stage);
+    return mcck == 1 ? scatter_kernel_bm<0, 1>(T, stage) : scatter_kernel_bm<0, 0>(T, stage);
+}
+
+// warp tiles.  abs: the species records its absorbed slots (ions with secondary emission)
+template <int BC, bool ABS>
+sort_kernel_t scatter_kernel_wm(int mcck) {
+    if (mcck == 1) return k_push_scatter_w<BC, ABS, 1>;
+    if (mcck == 2) return k_push_scatter_w<BC, ABS, 2>;
+    return k_push_scatter_w<BC, ABS, 0>;
+}
+sort_kernel_t scatter_kernel_w(int bc, bool abs, int mcck) {
+    if (bc == 1) return scatter_kernel_wm<1, false>(mcck);
+    return abs ? scatter_kernel_wm<0, true>(mcck) : scatter_kernel_wm<0, false>(mcck);
 }
 
 int occupancy_grid(pic1d* h, sort_kernel_t kernel, size_t smem) {
@@ -248,35 +298,37 @@ int occupancy_grid(pic1d* h, sort_kernel_t kernel, size_t smem) {
     return std::max(1, nb) * h->num_sms;
 }
 
+// per species two scatter kernels: [0] plain (the passes of a load sort nothing but particles), [1] the
+// step's (with the species' MCC folded in, unless PIC1D_FLAG_NO_FOLD)
 void setup_launch(pic1d* h) {
     cudaFuncSetAttribute(k_field_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, FIELD_SMEM_MAX * (int)sizeof(double));
-    cudaFuncSetAttribute(k_mcc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE_STAGE * sizeof(float)));
-    cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE_STAGE * sizeof(float)));
-    h->WA = std::min((h->n_sc + 1 + 3) / 4 * 4, PIC1D_WA_MAX);
+    h->WA = std::min((h->n_sc + 1 + 7) / 8 * 8, PIC1D_WA_MAX);
     h->smem_sort = (size_t)h->WA * sizeof(int);
     for (int s = 0; s < h->cfg.n_species; ++s) {
         SpeciesHost& p = h->sp[s];
         const bool abs = s == 1 && h->abs_list != nullptr;
-        if (p.warp_tiles) {
-            h->k_count[s] = h->cfg.bc == 1 ? k_push_count_w<1> : k_push_count_w<0>;
-            h->k_scatter[s] = h->cfg.bc == 1 ? k_push_scatter_w<1, false>
-                                             : (abs ? k_push_scatter_w<0, true> : k_push_scatter_w<0, false>);
-            h->smem_count[s] = 0;
-            h->smem_scatter[s] = 0;
-        } else {
-            const bool stage = s == 0;
-            h->k_count[s] = count_kernel(h->cfg.bc, h->T);
-            h->k_scatter[s] = scatter_kernel(h->cfg.bc, h->T, abs, stage);
-            h->smem_count[s] = h->smem_sort;
-            h->smem_scatter[s] = (size_t)h->WA * 9 * sizeof(unsigned) + (stage ? (size_t)h->T * 18 : 0);
+        for (int v = 0; v < 2; ++v) {
+            const int mcck = v ? p.mcck : 0;
+            if (p.warp_tiles) {
+                h->k_count[s] = h->cfg.bc == 1 ? k_push_count_w<1> : k_push_count_w<0>;
+                h->k_scatter[s][v] = scatter_kernel_w(h->cfg.bc, abs, mcck);
+                h->smem_count[s] = 0;
+                h->smem_scatter[s] = 0;
+            } else {
+                const bool stage = s == 0;
+                h->k_count[s] = count_kernel(h->cfg.bc, h->T);
+                h->k_scatter[s][v] = scatter_kernel(h->cfg.bc, h->T, stage, mcck);
+                h->smem_count[s] = h->smem_sort;
+                h->smem_scatter[s] = (size_t)h->WA * 4 + (stage ? std::max<size_t>((size_t)h->WA * 16, (size_t)h->T * 2) + (size_t)h->T * 18 : (size_t)h->WA * 16);
+            }
+            h->grid_scatter[s][v] = occupancy_grid(h, h->k_scatter[s][v], h->smem_scatter[s]);
         }
         h->grid_count[s] = occupancy_grid(h, h->k_count[s], h->smem_count[s]);
-        h->grid_scatter[s] = occupancy_grid(h, h->k_scatter[s], h->smem_scatter[s]);
     }
 }
 
-// fine sort of species s (mode 0: no push)
-void enqueue_sort(pic1d* h, int s, int shift = 0) {
+// fine sort of species s.  in_step: 1 = a regular step (push, folded MCC); 0 = a pass of a load's sort
+void enqueue_sort(pic1d* h, int s, int in_step, int shift = 0) {
     SpeciesHost& p = h->sp[s];
     SortArgs a = sort_args(h, s);
     if (shift > 0) {  // coarse pass of an unsorted load: sort by (sort cell >> shift)
@@ -285,27 +337,36 @@ void enqueue_sort(pic1d* h, int s, int shift = 0) {
     }
     const int tiles_per_block = p.warp_tiles ? PIC1D_NWARP : 1;
     const int nb_max = (p.n_tiles_max + tiles_per_block - 1) / tiles_per_block;
-    const int gc = std::min(h->grid_count[s], nb_max), gs = std::min(h->grid_scatter[s], nb_max);
+    const int gc = std::min(h->grid_count[s], nb_max), gs = std::min(h->grid_scatter[s][in_step], nb_max);
     h->k_count[s]<<<gc, PIC1D_NT, h->smem_count[s], h->stream>>>(a);
     mark(h, "push_count", s);
-    k_bin_scan<<<(a.n_sc + 31) / 32 + (a.abs_list ? 1 : 0), BINSCAN_NW * 32, 0, h->stream>>>(a);
+    const bool fold = in_step && p.mcck;
+    a.null_first = a.abs_list ? 1 : 0;
+    const int nb_null = fold ? (p.capacity / 32 + BINSCAN_NW * 32 - 1) / (BINSCAN_NW * 32) : 0;
+    k_bin_scan<<<(a.n_sc + 31) / 32 + a.null_first + nb_null, BINSCAN_NW * 32, 0, h->stream>>>(a);
     mark(h, "bin_scan", s);
     k_offsets_scan<<<1, 1024, 0, h->stream>>>(a);
     mark(h, "offsets_scan", s);
-    h->k_scatter[s]<<<gs, PIC1D_NT, h->smem_scatter[s], h->stream>>>(a);
+    h->k_scatter[s][in_step]<<<gs, PIC1D_NT, h->smem_scatter[s], h->stream>>>(a);
     mark(h, "push_scatter", s);
     p.cur ^= 1;
 }
 
 void enqueue_begin(pic1d* h, int mode) {
     const int ns = h->cfg.n_species;
-    k_step_begin<<<4, 256, 0, h->stream>>>(h->st, ns, mode, h->sp[0].T, ns > 1 ? h->sp[1].T : 0, h->sp[0].grp_lo, h->sp[0].grp_hi,
-                                           ns > 1 ? h->sp[1].grp_lo : nullptr, ns > 1 ? h->sp[1].grp_hi : nullptr,
-                                           h->sp[0].n_groups_max, ns > 1 ? h->sp[1].n_groups_max : 0);
+    BeginArgs b;
+    memset(&b, 0, sizeof(b));
+    b.st = h->st; b.n_species = ns; b.mode = mode;
+    for (int s = 0; s < ns; ++s) {
+        b.T[s] = h->sp[s].T; b.grp_lo[s] = h->sp[s].grp_lo; b.grp_hi[s] = h->sp[s].grp_hi;
+        b.n_groups[s] = h->sp[s].n_groups_max;
+    }
+    b.ion_nb = h->ion_nb; b.n_ion_nb = h->ion_nb ? h->sp[0].n_mcc_tiles : 0;
+    k_step_begin<<<4, 256, 0, h->stream>>>(b);
     mark(h, "step_begin", -1);
 }
 
-void enqueue_grid(pic1d* h, unsigned n_time) {
+void enqueue_grid(pic1d* h, int in_step) {
     const pic1d_config_t& c = h->cfg;
     CombineArgs cb;
     memset(&cb, 0, sizeof(cb));
@@ -325,7 +386,7 @@ void enqueue_grid(pic1d* h, unsigned n_time) {
     FieldArgs f;
     f.rho = h->rho; f.phi = h->phi; f.E = h->E; f.S = h->S; f.Tt = h->Tt; f.E32 = h->E32;
     f.Nc = c.n_cells; f.nodes = h->nodes; f.bc = c.bc; f.V0 = c.V0_norm; f.omega_dt = c.omega_dt;
-    f.n_time = n_time;
+    f.st = h->st; f.in_step = in_step;
     if (c.n_cells <= FIELD_SMEM_MAX) {
         const size_t sm = (size_t)((c.n_cells + 1023) / 1024) * 32 * 32 * sizeof(double);
         k_field_smem<<<1, 1024, sm, h->stream>>>(f);
@@ -335,54 +396,43 @@ void enqueue_grid(pic1d* h, unsigned n_time) {
     mark(h, "field", -1);
 }
 
+MccArgs mcc_args(pic1d* h, int s) {
+    const pic1d_config_t& c = h->cfg;
+    SpeciesHost& p = h->sp[s];
+    SpeciesHost& pe = h->sp[0];
+    MccArgs m;
+    memset(&m, 0, sizeof(m));
+    m.x = p.buf[p.cur][0]; m.vx = p.buf[p.cur][1]; m.vy = p.buf[p.cur][2]; m.vz = p.buf[p.cur][3];
+    m.ex = pe.buf[pe.cur][0]; m.evx = pe.buf[pe.cur][1]; m.evy = pe.buf[pe.cur][2]; m.evz = pe.buf[pe.cur][3];
+    m.cap_e = pe.capacity;
+    if (c.n_species > 1) {
+        SpeciesHost& pi = h->sp[1];
+        m.ix = pi.buf[pi.cur][0]; m.ivx = pi.buf[pi.cur][1]; m.ivy = pi.buf[pi.cur][2]; m.ivz = pi.buf[pi.cur][3];
+        m.cap_i = pi.capacity;
+    }
+    m.m = mcc_params(h, s);
+    m.n_species = c.n_species;
+    return m;
+}
+
+// the collisions that are not folded into a scatter, and the ionisation pairs
 void enqueue_mcc(pic1d* h) {
     const pic1d_config_t& c = h->cfg;
     for (int s = 0; s < c.n_species; ++s) {
-        if (c.sp[s].mcc_kind == 0) continue;
+        const int kind = c.sp[s].mcc_kind;
+        if (kind == 0) continue;
         SpeciesHost& p = h->sp[s];
-        SpeciesHost& pe = h->sp[0];
-        MccArgs m;
-        memset(&m, 0, sizeof(m));
-        m.x = p.buf[p.cur][0]; m.vx = p.buf[p.cur][1]; m.vy = p.buf[p.cur][2]; m.vz = p.buf[p.cur][3];
-        m.ex = pe.buf[pe.cur][0]; m.evx = pe.buf[pe.cur][1]; m.evy = pe.buf[pe.cur][2]; m.evz = pe.buf[pe.cur][3];
-        m.cap_e = pe.capacity;
-        if (c.n_species > 1) {
-            SpeciesHost& pi = h->sp[1];
-            m.ix = pi.buf[pi.cur][0]; m.ivx = pi.buf[pi.cur][1]; m.ivy = pi.buf[pi.cur][2]; m.ivz = pi.buf[pi.cur][3];
-            m.cap_i = pi.capacity;
-        }
-        m.st = h->st; m.mask = p.mask;
-        // ionisation records: per-tile counts + (slot, speed) lists in the electrons' INACTIVE buffer, which
-        // is scratch until the next step's scatter writes into it
-        m.rec_nb = reinterpret_cast<int*>(p.desc);
-        m.rec_rel = reinterpret_cast<int*>(pe.buf[pe.cur ^ 1][2]);
-        m.rec_gp = pe.buf[pe.cur ^ 1][3];
-        m.s = s; m.kind = c.sp[s].mcc_kind; m.n_species = c.n_species;
-        m.step = h->step; m.k0 = (uint32_t)c.seed; m.k1 = (uint32_t)(c.seed >> 32);
-        m.P0 = (float)c.sp[s].P0; m.inv_g_cap = (float)c.sp[s].inv_g_cap; m.c_eV = (float)c.sp[s].c_eV;
-        m.r_el = (float)c.r_el; m.r_exc = (float)c.r_exc; m.r_ion = (float)c.r_ion;
-        m.E_exc = (float)c.E_exc; m.E_ion = (float)c.E_ion;
-        m.two_mr = (float)(2.0 * c.mass_ratio); m.gvt = (float)c.gas_vth_ion;
-        // null test in integers: U(w) = (w >> 8) 2^-24 < P0  <=>  (w >> 8) < ceil(P0 2^24)  <=>  w <= null_le
-        const uint64_t thr = (uint64_t)std::ceil((double)m.P0 * 16777216.0) << 8;
-        m.null_any = thr > 0;
-        m.null_le = (uint32_t)(thr - 1);
-        const int grid = std::min(p.n_mcc_tiles, h->num_sms * 4);
-        // STAGE (velocities streamed into shared memory during the null test) is compiled but not selected:
-        // measured 0.624 ms staged (3 blocks/SM) vs 0.610 ms unstaged (4 blocks/SM) for config-4 electrons
-        const bool stage = false;
-        if (m.kind == 1) {
-            if (stage) k_mcc<1, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE_STAGE * sizeof(float), h->stream>>>(m);
-            else k_mcc<1, false><<<grid, PIC1D_NT, 0, h->stream>>>(m);
+        MccArgs m = mcc_args(h, s);
+        if (p.mcck == 0) {
+            const int grid = std::min(p.n_mcc_tiles, h->num_sms * 4);
+            if (kind == 1) k_mcc<1><<<grid, PIC1D_NT, 0, h->stream>>>(m);
+            else k_mcc<2><<<grid, PIC1D_NT, 0, h->stream>>>(m);
             mark(h, "mcc", s);
+        }
+        if (kind == 1) {
             k_mcc_births<<<h->num_sms, PIC1D_NT, 0, h->stream>>>(m);
             mark(h, "mcc_births", s);
-            continue;
-        } else {
-            if (stage) k_mcc<2, true><<<std::min(p.n_mcc_tiles, h->num_sms * 3), PIC1D_NT, 3 * MCC_TILE_STAGE * sizeof(float), h->stream>>>(m);
-            else k_mcc<2, false><<<grid, PIC1D_NT, 0, h->stream>>>(m);
         }
-        mark(h, "mcc", s);
     }
 }
 
@@ -390,7 +440,7 @@ void enqueue_step(pic1d* h) {
     const pic1d_config_t& c = h->cfg;
     enqueue_begin(h, 1);
     if (c.n_species > 1) {
-        enqueue_sort(h, 1);
+        enqueue_sort(h, 1, 1);
         if (h->abs_list) {
             SpeciesHost& pe = h->sp[0];
             SeeArgs sa;
@@ -398,13 +448,13 @@ void enqueue_step(pic1d* h) {
             sa.ex = pe.buf[pe.cur][0]; sa.evx = pe.buf[pe.cur][1]; sa.evy = pe.buf[pe.cur][2]; sa.evz = pe.buf[pe.cur][3];
             sa.cap_e = pe.capacity; sa.T = pe.T;
             sa.gamma = (float)c.see_gamma; sa.vth = (float)c.see_vth; sa.fNc = (float)c.n_cells;
-            sa.k0 = (uint32_t)c.seed; sa.k1 = (uint32_t)(c.seed >> 32); sa.step = h->step;
+            sa.k0 = (uint32_t)c.seed; sa.k1 = (uint32_t)(c.seed >> 32);
             k_see_emit<<<1, 1024, 0, h->stream>>>(sa);
             mark(h, "see_emit", 0);
         }
     }
-    enqueue_sort(h, 0);
-    enqueue_grid(h, h->step + 1u);
+    enqueue_sort(h, 0, 1);
+    enqueue_grid(h, 1);
     enqueue_mcc(h);
     h->step += 1u;
 }
@@ -414,7 +464,6 @@ int sticky_code(unsigned err) {
     if (err & ERRBIT_CAPACITY) return PIC1D_ERR_CAPACITY;
     if (err & ERRBIT_WORKSPACE) return PIC1D_ERR_WORKSPACE;
     if (err & ERRBIT_BADLOAD) return PIC1D_ERR_ARG;
-    if (err & ERRBIT_ORDER) return PIC1D_ERR_ORDER;
     return PIC1D_OK;
 }
 
@@ -429,7 +478,7 @@ __global__ void k_set_count(DevState* st, int s, int n) {
     memset(&sp, 0, sizeof(sp));
     sp.n_live = n;
 }
-__global__ void k_clear_err(DevState* st) { st->err = 0; st->step = 0; st->n_abs = 0; }
+__global__ void k_clear_err(DevState* st) { st->err = 0; st->step = 0; st->step_next = 0; st->n_abs = 0; }
 
 }  // namespace
 
@@ -469,8 +518,10 @@ int pic1d_create(const pic1d_config_t* cfg, void* workspace, size_t workspace_by
     h->last_err = cudaSuccess;
     // zero the bookkeeping (state, look-back descriptors); particle arrays need no initialisation
     bool ok = ck(h, cudaMemsetAsync(h->st, 0, sizeof(DevState), h->stream));
-    for (int s = 0; s < cfg->n_species && ok; ++s)
-        ok = ck(h, cudaMemsetAsync(h->sp[s].desc, 0, sizeof(ull) * h->sp[s].n_mcc_tiles, h->stream));
+    if (h->ion_bits) {
+        ok = ok && ck(h, cudaMemsetAsync(h->ion_bits, 0, sizeof(unsigned) * h->n_ion_words, h->stream));
+        ok = ok && ck(h, cudaMemsetAsync(h->ion_nb, 0, sizeof(int) * h->sp[0].n_mcc_tiles, h->stream));
+    }
     ok = ok && ck(h, cudaMemsetAsync(h->E32, 0, sizeof(float) * (h->nodes + 1), h->stream));
     if (!ok || !ck(h, cudaGetLastError())) { delete h; return PIC1D_ERR_CUDA; }
     *out = h;
@@ -512,7 +563,6 @@ int pic1d_load_particles(pic1d_t* h, int s, int64_t n, const float* x, const flo
     h->step = 0;
     for (int q = 0; q < h->cfg.n_species; ++q) {
         SpeciesHost& pq = h->sp[q];
-        cudaMemsetAsync(pq.desc, 0, sizeof(ull) * pq.n_mcc_tiles, h->stream);
         if (pq.mask) cudaMemsetAsync(pq.mask, 0, pq.capacity, h->stream);
     }
     // An unsorted load has full-width tile windows, wider than a tile's fixed pool row.  Sort by the
@@ -533,10 +583,10 @@ int pic1d_load_particles(pic1d_t* h, int s, int64_t n, const float* x, const flo
         for (int q = h->cfg.n_species - 1; q >= 0; --q) {
             const int pidx = r - (rounds - passes[q]);  // species with fewer passes join late
             if (pidx < 0) continue;
-            enqueue_sort(h, q, std::max(0, bits - (pidx + 1) * sb[q]));
+            enqueue_sort(h, q, 0, std::max(0, bits - (pidx + 1) * sb[q]));
         }
     }
-    enqueue_grid(h, 0u);
+    enqueue_grid(h, 0);
     if (!ck(h, cudaGetLastError())) return PIC1D_ERR_CUDA;
     if (!on_device && !ck(h, cudaStreamSynchronize(h->stream))) return PIC1D_ERR_CUDA;  // host buffers may go away
     h->ready = true;

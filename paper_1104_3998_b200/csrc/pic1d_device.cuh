@@ -8,7 +8,7 @@
 
 #define PIC1D_NT 256          // threads per block of the particle kernels
 #define PIC1D_NWARP (PIC1D_NT / 32)
-#define PIC1D_WA_MAX 1024     // bins of a tile window ranked at a time in shared memory (multiple of 4)
+#define PIC1D_WA_MAX 1920     // bins of a tile window ranked at a time in shared memory (multiple of 8)
 #define PIC1D_GROUP 64        // tiles per tile-group (window union used by the bin scan)
 
 // Philox stream ids (R12)
@@ -21,7 +21,6 @@
 #define ERRBIT_NONFINITE 2u
 #define ERRBIT_WORKSPACE 4u
 #define ERRBIT_BADLOAD 8u
-#define ERRBIT_ORDER 16u  // rank self-check failed (PIC1D_FLAG_VERIFY_ORDER)
 
 typedef unsigned long long ull;
 
@@ -43,10 +42,10 @@ struct DevSpecies {
 
 struct DevState {
     DevSpecies sp[2];
-    unsigned int step;  // n: index of the step being computed
-    unsigned int err;   // sticky ERRBIT_*
-    int n_abs;          // absorbed ions recorded in the list this step
-    int pad;
+    unsigned int step;       // n: index of the step being computed (set by k_step_begin)
+    unsigned int err;        // sticky ERRBIT_*
+    int n_abs;               // absorbed ions recorded in the list this step
+    unsigned int step_next;  // index the next step will get
 };
 
 // Philox4x32-10 (Salmon et al., SC'11).  key = (seed_lo, seed_hi).

@@ -198,7 +198,8 @@ struct FieldArgs {
     float* E32;
     int Nc, nodes, bc;
     double V0, omega_dt;
-    unsigned n_time;
+    const DevState* st;  // in_step: the wall potential is taken at t_{n+1}, n = st->step (device-resident)
+    int in_step;         // 0: t = 0 (right after a load)
 };
 
 __device__ double block_sum_d(double v) {
@@ -264,7 +265,7 @@ __global__ void __launch_bounds__(1024) k_field(FieldArgs a) {
     block_inclusive_scan_d([=](int i) { return i == 0 ? 0.0 : rho[i] - mean; }, a.S, N);
     const double* S = a.S;
     block_inclusive_scan_d([=](int i) { return S[i]; }, a.Tt, N);
-    const double phi0 = a.bc == 0 ? a.V0 * sin(a.omega_dt * (double)a.n_time) : 0.0;
+    const double phi0 = a.bc == 0 ? a.V0 * sin(a.omega_dt * (double)(a.in_step ? a.st->step + 1u : 0u)) : 0.0;
     const double phiN = 0.0;
     const double d1 = (phiN - phi0 + a.Tt[N - 1]) / (double)N;
     double psum = 0.0;
@@ -349,7 +350,7 @@ __global__ void __launch_bounds__(1024) k_field_smem(FieldArgs a) {
     // scan 2 (T_j = sum_{i<=j} S_i) fused with the outputs
     double toff = 0.0, T_all = 0.0;
     for (int q = 0; q < 32; ++q) { const double v = s_w[q]; if (q < wp) toff += v; T_all += v; }
-    const double phi0 = a.bc == 0 ? a.V0 * sin(a.omega_dt * (double)a.n_time) : 0.0;
+    const double phi0 = a.bc == 0 ? a.V0 * sin(a.omega_dt * (double)(a.in_step ? a.st->step + 1u : 0u)) : 0.0;
     const double phiN = 0.0;
     const double d1 = (phiN - phi0 + T_all) / (double)N;  // T_all = T_{N-1}
     double psum = 0.0, carry = toff;

@@ -20,6 +20,7 @@
 // breaks when they do not (configs 2-4 electrons), the window just gets wider.
 #pragma once
 #include "pic1d_device.cuh"
+#include "pic1d_mcc.cuh"
 
 struct SortArgs {
     const float *sx, *svx, *svy, *svz;  // source buffer
@@ -41,8 +42,9 @@ struct SortArgs {
     float kappa, fNc, inv_r;
     int Nc, n_sc;
     int shift;  // key = sort cell >> shift (0 except in the coarse pass of an unsorted load)
-    int WA;     // sub-window (bins) the scatter kernel ranks at a time in shared memory
-    int verify; // self-check of the rank order (debug)
+    int WA;     // sub-window (bins) the scatter kernel ranks at a time in shared memory (a multiple of 8)
+    MccP m;     // collision model of the species, for the scatter kernels that fold the MCC in
+    int null_first;  // k_bin_scan: blocks from (bin blocks + null_first) on compute the null-test bit mask
 };
 
 // ---- pass 1 -----------------------------------------------------------------------------------
@@ -258,7 +260,14 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
     __shared__ int s_part[BINSCAN_NW][33];
     __shared__ int4 s_desc[BINSCAN_DESC];
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
-    if (blockIdx.x * 32 >= a.n_sc) {
+    const int nb_bins = (a.n_sc + 31) / 32;
+    if ((int)blockIdx.x >= nb_bins + a.null_first) {
+        // extra blocks (species whose MCC is folded into the scatter): the null-test bit mask of this step,
+        // 1024 words = 32768 slots per block, concurrently with the bin blocks
+        mcc_null_words(a.m, ((int)blockIdx.x - nb_bins - a.null_first) * (BINSCAN_NW * 32) + tid);
+        return;
+    }
+    if ((int)blockIdx.x >= nb_bins) {
         // one extra block (species with an ordered absorbed list only): exclusive prefix of the per-tile
         // absorbed counts, concurrently with the bin blocks
         DevSpecies& sp = a.st->sp[a.s];
@@ -423,12 +432,14 @@ __global__ void __launch_bounds__(1024) k_offsets_scan(SortArgs a) {
 // so the blocks advance through the source as one narrow front and the destination lines they share
 // meet in L2.
 //
-// Stable rank inside the tile without any serial section: every warp owns ROWS*32 consecutive slots
-// and a private 32-bit counter per bin of the tile's window.  A shared-memory atomicAdd returns the
-// rank inside the warp's segment: rows are issued in slot order, and lanes of one instruction that
-// hit the same counter are served in ascending lane order (measured on sm_100a, DESIGN.md "Kernels";
-// a.verify re-checks it with match.any and raises a sticky error).  A per-bin pass (4 bins per
-// thread, 128-bit shared accesses) then turns the 8 per-warp counts into per-warp bases, and
+// Stable rank inside the tile without any serial section and without any atomic: every warp owns
+// ROWS*32 consecutive slots and a private 16-bit counter per bin of the tile's window (a warp holds at
+// most 256 particles of a bin).  Per row, match.any groups the lanes with equal keys; the lowest lane of
+// a group reads and advances the warp's counter of that bin, the others take counter + (number of lower
+// lanes with the same key).  Rows are taken in slot order, so the rank is the particle's position among
+// the warp's particles of that bin BY CONSTRUCTION (no assumption about the order in which the hardware
+// serves conflicting shared-memory atomics).  A per-bin pass (8 bins per thread, 128-bit shared accesses
+// on packed 16-bit pairs) then turns the 8 per-warp counts into per-warp bases, and
 //     destination = offsets[k] + prefix over earlier tiles [t][k] + prefix over earlier warps + rank.
 // Only x and vx are loaded up front (the push and the key need nothing else); vy and vz are fetched
 // after the ranks are known, so their latency overlaps the per-bin pass and fewer registers are live.
@@ -437,25 +448,31 @@ __global__ void __launch_bounds__(1024) k_offsets_scan(SortArgs a) {
 // particles move many cells per step, Eq. 5 violated), the per-bin pass also scans the bin totals,
 // the particles are first placed in tile-sorted order in shared memory and then copied out by
 // consecutive threads, so that a warp's store covers a few runs instead of 32 separate sectors.
-// ABS (ions with secondary emission): absorbed particles form a pseudo-bin after the window and are
-// written, in slot order, to the absorbed list.  Windows wider than WA bins are ranked WA bins at a
-// time (direct scatter).
-template <int BC, int ROWS, bool ABS, bool STAGE>
+// Windows wider than WA bins are ranked WA bins at a time (direct scatter).
+//
+// MCCK != 0: the null-collision MCC of the species is folded in (mcc_lane, pic1d_mcc.cuh): the
+// destination slot is the particle id, and the velocities are at hand -- in registers on the direct
+// path, in the staging buffer on the staged path.
+template <int BC, int ROWS, bool STAGE, int MCCK>
 __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k_push_scatter(SortArgs a) {
     extern __shared__ unsigned s_mem[];
     __shared__ int s_tile;
+    __shared__ int s_n[2];           // MCCK: candidates, real collisions of the tile
     __shared__ unsigned s_scan[PIC1D_NWARP + 1];
-    const int WA = a.WA;             // a multiple of 4
-    unsigned* s_base = s_mem;        // [WA] absolute destination of the tile's first particle per bin
-    unsigned* s_cnt = s_mem + WA;    // [8][WA] per-warp counters, then per-warp bases
+    const int WA = a.WA;             // a multiple of 8
     constexpr int T = PIC1D_NT * ROWS;
-    float* s_st = reinterpret_cast<float*>(s_mem + 9 * WA);                   // STAGE: [4][T]
+    unsigned* s_base = s_mem;        // [WA] absolute destination of the tile's first particle per bin
+    unsigned short* s_cnt = reinterpret_cast<unsigned short*>(s_mem + WA);  // [8][WA] per-warp counters, then bases
+    const int cnt_words = (STAGE && MCCK) ? max(4 * WA, T / 2) : 4 * WA;      // (the MCC list needs T shorts)
+    float* s_st = reinterpret_cast<float*>(s_mem + WA + cnt_words);           // STAGE: [4][T]
     unsigned short* s_key = reinterpret_cast<unsigned short*>(s_st + 4 * T);  // STAGE: [T]
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
-    unsigned* my = s_cnt + wp * WA;
+    unsigned short* my = s_cnt + wp * WA;
     DevSpecies& sp = a.st->sp[a.s];
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
-    for (int i = tid; i < 8 * WA; i += PIC1D_NT) s_cnt[i] = 0u;  // counters are zero between tiles
+    const uint32_t step = a.st->step;
+    MccCount mc = {0u, 0u, 0u};
+    for (int i = tid; i < cnt_words; i += PIC1D_NT) reinterpret_cast<unsigned*>(s_cnt)[i] = 0u;  // counters are zero between tiles
     if (tid == 0) s_tile = atomicAdd(&sp.ticket2, 1);
     __syncthreads();
     while (true) {
@@ -464,10 +481,9 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
         const int lo = a.tile_lo[tile], w = a.tile_w[tile], off = a.tile_off[tile];
         const int base = tile * T + wp * (ROWS * 32) + lane;
         const bool full = tile * T + T <= n_push;  // block-uniform
-        const int wtot = off < 0 ? 0 : (ABS ? w + 1 : w);  // off < 0: count pool exhausted (sticky error), drop the tile
+        const int wtot = off < 0 ? 0 : w;          // off < 0: count pool exhausted (sticky error), the tile is lost
         float x[ROWS], vx[ROWS], vy[ROWS], vz[ROWS];
-        int rel[ROWS];  // bin relative to the window; w = absorbed (ABS); -1 = no particle / done
-        unsigned wall = 0;
+        int rel[ROWS];  // bin relative to the window; -1 = no particle / done
         if (full) {
 #pragma unroll
             for (int r = 0; r < ROWS; ++r) { x[r] = __ldcs(a.sx + base + r * 32); vx[r] = __ldcs(a.svx + base + r * 32); }
@@ -481,43 +497,41 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
         }
         // absolute base of the tile per bin of the first sub-window: in flight together with the particles
         for (int i = tid; i < min(WA, wtot); i += PIC1D_NT)
-            s_base[i] = i < w ? (unsigned)(a.offsets[lo + i] + __ldcg(a.pool + off + i)) : (unsigned)a.tile_dead[tile];
+            s_base[i] = (unsigned)(a.offsets[lo + i] + __ldcg(a.pool + off + i));
+        int n_lost = 0;
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
             const int i = base + r * 32;
             rel[r] = -1;
             if (full || i < n_src) {
                 const int key = push_particle<BC>(x[r], vx[r], full || i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
-                rel[r] = key >= 0 ? key - lo : (ABS ? w : -1);
-                if (ABS && key == -2) wall |= 1u << r;
+                rel[r] = key >= 0 ? key - lo : -1;
+                n_lost += (off < 0 && key >= 0) ? 1 : 0;
             }
         }
-        const bool staged = STAGE && !ABS && wtot <= WA && wtot >= T / 64;  // block-uniform
+        if (off < 0) {  // block-uniform, after a sticky workspace error only: count what is lost
+            n_lost = __reduce_add_sync(0xffffffffu, n_lost);
+            if (lane == 0 && n_lost) atomicAdd(&sp.dropped, (ull)n_lost);
+        }
+        const bool staged = STAGE && wtot <= WA && wtot >= T / 64;  // block-uniform
         for (int sub = 0; sub < wtot; sub += WA) {
             const int nsub = min(WA, wtot - sub);
-            // ---- rank inside the warp's segment ---------------------------------------------------
+            // ---- rank inside the warp's segment: match.any groups, the group's lowest lane advances the counter
             unsigned ranked = 0;
 #pragma unroll
             for (int r = 0; r < ROWS; ++r) {
                 const int k = rel[r] - sub;
                 const bool in = rel[r] >= 0 && k < nsub;  // rel < sub only for particles already scattered (-1)
-                const int k0 = __shfl_sync(0xffffffffu, k, 0);
-                if (__all_sync(0xffffffffu, in && k == k0)) {
-                    unsigned old = 0;
-                    if (lane == 0) old = atomicAdd(&my[k0], 32u);
-                    old = __shfl_sync(0xffffffffu, old, 0);
-                    rel[r] = k | ((int)(old + lane) << 16);
-                    ranked |= 1u << r;
-                } else if (in) {
-                    const int rank = (int)atomicAdd(&my[k], 1u);
-                    if (a.verify) {
-                        const unsigned peers = __match_any_sync(__activemask(), k);
-                        const int first = __shfl_sync(peers, rank, __ffs(peers) - 1);
-                        if (rank != first + __popc(peers & lanemask_lt())) atomicOr(&a.st->err, ERRBIT_ORDER);
-                    }
-                    rel[r] = k | (rank << 16);
+                const unsigned peers = __match_any_sync(0xffffffffu, in ? k : (0x40000000 | lane));
+                const int leader = __ffs(peers) - 1;
+                unsigned old = 0;
+                if (in && lane == leader) { old = my[k]; my[k] = (unsigned short)(old + __popc(peers)); }
+                old = __shfl_sync(0xffffffffu, old, leader);
+                if (in) {
+                    rel[r] = k | ((int)(old + __popc(peers & lanemask_lt())) << 16);
                     ranked |= 1u << r;
                 }
+                __syncwarp();  // the next row's leaders see the advanced counters
             }
             if (sub == 0) {  // payload: needed only for the stores
                 if (full) {
@@ -533,25 +547,26 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
                 }
             }
             __syncthreads();
-            // ---- per bin: counts of the 8 warps -> bases of the 8 warps ------------------------------
-            // direct: base = absolute destination; staged: base = position in the tile-sorted order,
+            // ---- per bin: counts of the 8 warps -> prefix over earlier warps (16-bit pairs packed in 32-bit words)
+            // direct: s_cnt = prefix over earlier warps; staged: s_cnt = position in the tile-sorted order,
             // and s_base becomes (absolute destination - position of the bin's first particle)
             unsigned n_out = 0;
-            for (int c0 = 0; c0 < nsub; c0 += 4 * PIC1D_NT) {  // 1024 bins per round, in bin order
-                const int i4 = c0 + tid * 4;
-                const bool act = i4 < nsub;
+            for (int c0 = 0; c0 < nsub; c0 += 8 * PIC1D_NT) {  // 2048 bins per round, in bin order
+                const int i8 = c0 + tid * 8;
+                const bool act = i8 < nsub;
                 uint4 tot = make_uint4(0u, 0u, 0u, 0u);
                 if (act) {
 #pragma unroll
                     for (int q = 0; q < PIC1D_NWARP; ++q) {
-                        const uint4 c = *reinterpret_cast<const uint4*>(s_cnt + q * WA + i4);
+                        const uint4 c = *reinterpret_cast<const uint4*>(s_cnt + q * WA + i8);
                         tot.x += c.x; tot.y += c.y; tot.z += c.z; tot.w += c.w;
                     }
                 }
-                uint4 b4 = make_uint4(0u, 0u, 0u, 0u);
-                if (act) b4 = *reinterpret_cast<const uint4*>(s_base + i4);
+                uint4 b4 = make_uint4(0u, 0u, 0u, 0u);  // packed start per bin
                 if (staged) {  // block-wide exclusive scan of the bin totals
-                    const unsigned S = tot.x + tot.y + tot.z + tot.w;
+                    const unsigned t0 = tot.x & 0xffffu, t1 = tot.x >> 16, t2 = tot.y & 0xffffu, t3 = tot.y >> 16,
+                                   t4 = tot.z & 0xffffu, t5 = tot.z >> 16, t6 = tot.w & 0xffffu, t7 = tot.w >> 16;
+                    const unsigned S = t0 + t1 + t2 + t3 + t4 + t5 + t6 + t7;
                     unsigned inc = S;
 #pragma unroll
                     for (int o = 1; o < 32; o <<= 1) {
@@ -566,34 +581,43 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
                     for (int q = 0; q < PIC1D_NWARP; ++q) { const unsigned v = s_scan[q]; if (q < wp) before += v; all += v; }
                     const unsigned e0 = n_out + before + inc - S;
                     n_out += all;
-                    const uint4 ls = make_uint4(e0, e0 + tot.x, e0 + tot.x + tot.y, e0 + tot.x + tot.y + tot.z);
-                    if (act)
-                        *reinterpret_cast<uint4*>(s_base + i4) = make_uint4(b4.x - ls.x, b4.y - ls.y, b4.z - ls.z, b4.w - ls.w);
-                    b4 = ls;
+                    const unsigned e1 = e0 + t0, e2 = e1 + t1, e3 = e2 + t2, e4 = e3 + t3, e5 = e4 + t4, e6 = e5 + t5, e7 = e6 + t6;
+                    if (act) {
+                        uint4 lo4 = *reinterpret_cast<const uint4*>(s_base + i8);
+                        uint4 hi4 = *reinterpret_cast<const uint4*>(s_base + i8 + 4);
+                        lo4.x -= e0; lo4.y -= e1; lo4.z -= e2; lo4.w -= e3;
+                        hi4.x -= e4; hi4.y -= e5; hi4.z -= e6; hi4.w -= e7;
+                        *reinterpret_cast<uint4*>(s_base + i8) = lo4;
+                        *reinterpret_cast<uint4*>(s_base + i8 + 4) = hi4;
+                    }
+                    b4 = make_uint4(e0 | (e1 << 16), e2 | (e3 << 16), e4 | (e5 << 16), e6 | (e7 << 16));
                 }
                 if (act) {
 #pragma unroll
                     for (int q = 0; q < PIC1D_NWARP; ++q) {  // counts are re-read: keeping them would spill
-                        const uint4 c = *reinterpret_cast<const uint4*>(s_cnt + q * WA + i4);
-                        *reinterpret_cast<uint4*>(s_cnt + q * WA + i4) = b4;
+                        const uint4 c = *reinterpret_cast<const uint4*>(s_cnt + q * WA + i8);
+                        *reinterpret_cast<uint4*>(s_cnt + q * WA + i8) = b4;
                         b4.x += c.x; b4.y += c.y; b4.z += c.z; b4.w += c.w;
                     }
                 }
             }
             __syncthreads();
             if (!staged) {
-                // ---- direct scatter: destination = base of (warp, bin) + rank in the warp ------------
+                // ---- direct scatter: destination = tile's base of the bin + prefix over earlier warps + rank
 #pragma unroll
                 for (int r = 0; r < ROWS; ++r) {
-                    if (!((ranked >> r) & 1u)) continue;
+                    const bool act = (ranked >> r) & 1u;
                     const int k = rel[r] & 0xffff;
-                    const unsigned d = my[k] + (unsigned)(rel[r] >> 16);
-                    if (!ABS || sub + k < w) {
-                        a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
-                    } else if (a.abs_list && (int)d < a.abs_cap) {  // absorbed: ordered list of (slot, wall)
-                        a.abs_list[d] = (unsigned)(base + r * 32) | (((wall >> r) & 1u) << 31);
+                    unsigned d = 0;
+                    if (act) d = s_base[k] + (unsigned)my[k] + (unsigned)(rel[r] >> 16);
+                    if (MCCK) {
+                        const int e = mcc_lane<MCCK>(a.m, step, d, act && mcc_null_bit(a.m, d), vx[r], vy[r], vz[r], mc);
+                        if (a.m.mask && act) a.m.mask[d] = (uint8_t)e;
                     }
-                    rel[r] = -1;
+                    if (act) {
+                        a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
+                        rel[r] = -1;
+                    }
                 }
             } else {
                 // ---- staged: tile-sorted order in shared memory, then coalesced copy-out ----------------
@@ -601,29 +625,78 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
                 for (int r = 0; r < ROWS; ++r) {
                     if (!((ranked >> r) & 1u)) continue;
                     const int k = rel[r] & 0xffff;
-                    const unsigned li = my[k] + (unsigned)(rel[r] >> 16);
+                    const unsigned li = (unsigned)my[k] + (unsigned)(rel[r] >> 16);
                     s_st[li] = x[r]; s_st[T + li] = vx[r]; s_st[2 * T + li] = vy[r]; s_st[3 * T + li] = vz[r];
                     s_key[li] = (unsigned short)k;
                     rel[r] = -1;
                 }
+                if (MCCK && tid == 0) s_n[1] = 0;
                 __syncthreads();
-                for (int j = tid; j < (int)n_out; j += PIC1D_NT) {
-                    const unsigned d = s_base[s_key[j]] + (unsigned)j;
-                    a.dx[d] = s_st[j]; a.dvx[d] = s_st[T + j]; a.dvy[d] = s_st[2 * T + j]; a.dvz[d] = s_st[3 * T + j];
+                if (!MCCK) {
+                    for (int j = tid; j < (int)n_out; j += PIC1D_NT) {
+                        const unsigned d = s_base[s_key[j]] + (unsigned)j;
+                        a.dx[d] = s_st[j]; a.dvx[d] = s_st[T + j]; a.dvy[d] = s_st[2 * T + j]; a.dvz[d] = s_st[3 * T + j];
+                    }
+                } else {
+                    // The collisions, folded in: the destination slot is the particle id, the velocities are in
+                    // the staging buffer.  Copy-out and null-test look-ups of the whole tile first (all in flight
+                    // together), then the process selection of the candidates, row by row; the real collisions go
+                    // to a list (the per-warp counters are free by now and hold it) ...
+                    unsigned short* s_rl = s_cnt;  // [T] real collisions: j | event << 12
+                    unsigned dj[ROWS], nw[ROWS];
+#pragma unroll
+                    for (int it = 0; it < ROWS; ++it) {
+                        const int j = it * PIC1D_NT + tid;
+                        dj[it] = 0u; nw[it] = 0u;
+                        if (j < (int)n_out) {
+                            const unsigned d = s_base[s_key[j]] + (unsigned)j;
+                            dj[it] = d;
+                            nw[it] = __ldcg(a.m.null_bits + (d >> 5));
+                            a.dx[d] = s_st[j]; a.dvx[d] = s_st[T + j]; a.dvy[d] = s_st[2 * T + j]; a.dvz[d] = s_st[3 * T + j];
+                            if (a.m.mask) a.m.mask[d] = 0;
+                        }
+                    }
+#pragma unroll
+                    for (int it = 0; it < ROWS; ++it) {
+                        const int j = it * PIC1D_NT + tid;
+                        const unsigned d = dj[it];
+                        const bool cand = j < (int)n_out && ((nw[it] >> (d & 31u)) & 1u);
+                        if (!__any_sync(0xffffffffu, cand)) continue;
+                        uint32_t b0[4];
+                        const int e = mcc_event<MCCK>(a.m, step, d, cand, s_st[T + j], s_st[2 * T + j], s_st[3 * T + j], mc, b0);
+                        if (a.m.mask && e) a.m.mask[d] = (uint8_t)e;
+                        const int idx = warp_append(e != 0, &s_n[1]);
+                        if (e) s_rl[idx] = (unsigned short)(j | (e << 12));
+                    }
+                    __syncthreads();
+                    // ... and get their kinematics one thread per real collision
+                    const int n_coll = s_n[1];
+                    for (int c = tid; c < n_coll; c += PIC1D_NT) {  // one thread per real collision: kinematics
+                        const int j = s_rl[c] & 0xfff, e = s_rl[c] >> 12;
+                        const unsigned d = s_base[s_key[j]] + (unsigned)j;
+                        uint32_t b0[4];
+                        philox4x32_10(d, step, STREAM_COLL + (uint32_t)a.m.s, 0u, a.m.k0, a.m.k1, b0);
+                        float cx = s_st[T + j], cy = s_st[2 * T + j], cz = s_st[3 * T + j];
+                        mcc_kinematics<MCCK>(a.m, step, d, e, b0, cx, cy, cz);
+                        a.dvx[d] = cx; a.dvy[d] = cy; a.dvz[d] = cz;  // overwrites the copy-out of this block
+                    }
                 }
             }
             __syncthreads();
             // ---- zero the counters again; next sub-window's bases ---------------------------------------
             {
-                for (int i4 = tid * 4; i4 < nsub; i4 += 4 * PIC1D_NT) {
+                if (MCCK && staged) {  // the collision list lay over the counters
+                    for (int i8 = tid * 8; i8 < T; i8 += 8 * PIC1D_NT)
+                        *reinterpret_cast<uint4*>(s_cnt + i8) = make_uint4(0u, 0u, 0u, 0u);
+                }
+                for (int i8 = tid * 8; i8 < nsub; i8 += 8 * PIC1D_NT) {
 #pragma unroll
                     for (int q = 0; q < PIC1D_NWARP; ++q)
-                        *reinterpret_cast<uint4*>(s_cnt + q * WA + i4) = make_uint4(0u, 0u, 0u, 0u);
+                        *reinterpret_cast<uint4*>(s_cnt + q * WA + i8) = make_uint4(0u, 0u, 0u, 0u);
                 }
                 for (int i = tid; i < nsub; i += PIC1D_NT) {
                     const int kk = sub + WA + i;
-                    if (kk < wtot)
-                        s_base[i] = kk < w ? (unsigned)(a.offsets[lo + kk] + __ldcg(a.pool + off + kk)) : (unsigned)a.tile_dead[tile];
+                    if (kk < wtot) s_base[i] = (unsigned)(a.offsets[lo + kk] + __ldcg(a.pool + off + kk));
                 }
             }
             if (sub + WA < wtot) __syncthreads();
@@ -631,29 +704,43 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
         if (tid == 0) s_tile = atomicAdd(&sp.ticket2, 1);
         __syncthreads();
     }
+    if (MCCK) mcc_flush_counts(a.m, mc);
 }
 
 // ---- set up the sorts of one step ------------------------------------------------------------------
-// mode 0: initial sort after a load (nothing is pushed); mode 1: a regular step.
-__global__ void k_step_begin(DevState* st, int n_species, int mode, int T0, int T1, int* grp_lo0, int* grp_hi0,
-                             int* grp_lo1, int* grp_hi1, int n_groups0, int n_groups1) {
-    const int tid = threadIdx.x + blockIdx.x * blockDim.x;
+// mode 0: initial sort after a load (nothing is pushed); mode 1: a regular step, which also advances the
+// device-resident step index (every kernel reads the step from DevState, never from a host argument, so
+// a captured CUDA graph of the step can be replayed).
+struct BeginArgs {
+    DevState* st;
+    int n_species, mode;
+    int T[2];
+    int *grp_lo[2], *grp_hi[2];
+    int n_groups[2];
+    int* ion_nb;   // per-MCC-tile ionisation counts of the electron set (may be null)
+    int n_ion_nb;
+};
+
+__global__ void k_step_begin(BeginArgs b) {
+    DevState* st = b.st;
+    const int tid = threadIdx.x + blockIdx.x * blockDim.x, nthr = blockDim.x * gridDim.x;
     if (tid == 0) {
-        for (int s = 0; s < n_species; ++s) {
+        for (int s = 0; s < b.n_species; ++s) {
             DevSpecies& sp = st->sp[s];
-            sp.n_push = mode ? sp.n_live : 0;
+            sp.n_push = b.mode ? sp.n_live : 0;
             sp.n_src = sp.n_live;
-            const int T = s == 0 ? T0 : T1;
-            sp.n_tiles = (sp.n_live + T - 1) / T;
+            sp.n_tiles = (sp.n_live + b.T[s] - 1) / b.T[s];
             sp.n_dead = 0;
             sp.pool_used = 0;
             sp.ticket = 0;
             sp.ticket2 = 0;
         }
         st->n_abs = 0;
+        if (b.mode) { st->step = st->step_next; st->step_next = st->step + 1u; }
     }
-    for (int i = tid; i < n_groups0; i += blockDim.x * gridDim.x) { grp_lo0[i] = 0x7fffffff; grp_hi0[i] = -1; }
-    for (int i = tid; i < n_groups1; i += blockDim.x * gridDim.x) { grp_lo1[i] = 0x7fffffff; grp_hi1[i] = -1; }
+    for (int s = 0; s < b.n_species; ++s)
+        for (int i = tid; i < b.n_groups[s]; i += nthr) { b.grp_lo[s][i] = 0x7fffffff; b.grp_hi[s][i] = -1; }
+    for (int i = tid; i < b.n_ion_nb; i += nthr) b.ion_nb[i] = 0;
 }
 
 // ---- secondary-electron emission at ion impact (L41; R19) --------------------------------
@@ -665,7 +752,7 @@ struct SeeArgs {
     int cap_e;
     int T;
     float gamma, vth, fNc;
-    uint32_t k0, k1, step;
+    uint32_t k0, k1;
 };
 
 __global__ void __launch_bounds__(1024) k_see_emit(SeeArgs a) {
@@ -679,7 +766,7 @@ __global__ void __launch_bounds__(1024) k_see_emit(SeeArgs a) {
         if (tid == 0) atomicOr(&st->err, ERRBIT_CAPACITY);
     }
     const int ne = st->sp[0].n_live;
-    const uint32_t step = a.step;
+    const uint32_t step = st->step;
     if (tid == 0) s_run = 0;
     __syncthreads();
     for (int base = 0; base < n_abs; base += 1024) {

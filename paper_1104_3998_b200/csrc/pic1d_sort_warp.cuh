@@ -138,7 +138,8 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count_w(SortArgs a) {
     }
 }
 
-template <int BC, bool ABS>
+// MCCK != 0: the species' null-collision MCC is folded in (mcc_lane: the destination slot is the particle id)
+template <int BC, bool ABS, int MCCK>
 __global__ void __launch_bounds__(PIC1D_NT, 4) k_push_scatter_w(SortArgs a) {
     __shared__ unsigned s_cur[PIC1D_NWARP][PIC1D_PSW + 1];  // next free destination per window bin (+ absorbed)
     constexpr int ROWS = PIC1D_TW / 32;
@@ -147,14 +148,19 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_push_scatter_w(SortArgs a) {
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
     const int n_warps = gridDim.x * PIC1D_NWARP;
     unsigned* cur = s_cur[wp];
+    const uint32_t step = a.st->step;
+    MccCount mc = {0u, 0u, 0u};
     for (int tile = blockIdx.x * PIC1D_NWARP + wp; tile < n_tiles; tile += n_warps) {
         const int lo = a.tile_lo[tile], w = a.tile_w[tile], off = a.tile_off[tile];
-        if (off < 0) continue;  // count pool exhausted (sticky error): drop the tile
+        if (off < 0) {  // count pool exhausted (sticky error): the tile is lost, and counted as dropped
+            if (lane == 0) atomicAdd(&sp.dropped, (ull)min(PIC1D_TW, n_src - tile * PIC1D_TW));
+            continue;
+        }
         const int base = tile * PIC1D_TW + lane;
         const bool full = tile * PIC1D_TW + PIC1D_TW <= n_push;  // warp-uniform
         const bool narrow = w <= PIC1D_PSW;
         float x[ROWS], vx[ROWS], vy[ROWS], vz[ROWS];
-        int k[ROWS];  // bin relative to the window; w = absorbed (ABS); -1 = no particle
+        int k[ROWS];  // bin relative to the window; w = absorbed (ABS); -1 = no particle; MCCK: then the destination
         unsigned wall = 0;
         if (full) {
 #pragma unroll
@@ -209,9 +215,12 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_push_scatter_w(SortArgs a) {
                 const unsigned d = old + __popc(peers & lanemask_lt());
                 if (kk >= 0) {
                     if (!ABS || kk < w) {
-                        a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
-                    } else if (a.abs_list && (int)d < a.abs_cap) {  // absorbed: ordered list of (slot, wall)
-                        a.abs_list[d] = (unsigned)(base + r * 32) | (((wall >> r) & 1u) << 31);
+                        if (!MCCK) { a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r]; }
+                        else k[r] = (int)d | (1 << 30);  // remember the slot (= particle id); stored below
+                    } else {
+                        if (a.abs_list && (int)d < a.abs_cap)  // absorbed: ordered list of (slot, wall)
+                            a.abs_list[d] = (unsigned)(base + r * 32) | (((wall >> r) & 1u) << 31);
+                        if (MCCK) k[r] = -1;
                     }
                 }
                 __syncwarp();  // the next row's leaders see the advanced cursors
@@ -235,13 +244,53 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_push_scatter_w(SortArgs a) {
                 const unsigned d = old + __popc(peers & lanemask_lt());
                 if (kk >= 0) {
                     if (!ABS || kk < w) {
-                        a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
-                    } else if (a.abs_list && (int)d < a.abs_cap) {
-                        a.abs_list[d] = (unsigned)(base + r * 32) | (((wall >> r) & 1u) << 31);
+                        if (!MCCK) { a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r]; }
+                        else k[r] = (int)d | (1 << 30);
+                    } else {
+                        if (a.abs_list && (int)d < a.abs_cap)
+                            a.abs_list[d] = (unsigned)(base + r * 32) | (((wall >> r) & 1u) << 31);
+                        if (MCCK) k[r] = -1;
                     }
                 }
                 __syncwarp();
             }
         }
+        if (MCCK) {
+            // All destinations are known: the stores and the null-test look-ups of the 8 rows go out together.
+            unsigned nw[ROWS];
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) {
+                nw[r] = 0u;
+                if (k[r] >= 0) {
+                    const unsigned d = (unsigned)k[r] & 0x3fffffffu;
+                    k[r] = (int)d;
+                    a.dx[d] = x[r]; a.dvx[d] = vx[r]; a.dvy[d] = vy[r]; a.dvz[d] = vz[r];
+                    nw[r] = __ldcg(a.m.null_bits + (d >> 5));
+                    if (a.m.mask) a.m.mask[d] = 0;
+                }
+            }
+            unsigned cmask = 0;  // rows whose particle passed the null test
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r)
+                if (k[r] >= 0 && ((nw[r] >> ((unsigned)k[r] & 31u)) & 1u)) cmask |= 1u << r;
+            // The tile's candidates (few: P0 of the particles), one per lane and round: selection,
+            // kinematics, and the collided velocity overwrites the one this lane has just stored.
+            while (__any_sync(0xffffffffu, cmask != 0u)) {
+                const bool has = cmask != 0u;
+                const int r = has ? __ffs(cmask) - 1 : 0;
+                cmask &= cmask - 1u;
+                unsigned d = 0;
+                float cx = 0.0f, cy = 0.0f, cz = 0.0f;
+#pragma unroll
+                for (int q = 0; q < ROWS; ++q)
+                    if (q == r) { d = (unsigned)k[q]; cx = vx[q]; cy = vy[q]; cz = vz[q]; }
+                const int e = mcc_lane<MCCK>(a.m, step, d, has, cx, cy, cz, mc);
+                if (e) {
+                    a.dvx[d] = cx; a.dvy[d] = cy; a.dvz[d] = cz;
+                    if (a.m.mask) a.m.mask[d] = (uint8_t)e;
+                }
+            }
+        }
     }
+    if (MCCK) mcc_flush_counts(a.m, mc);
 }

@@ -16,6 +16,8 @@ OK, ERR_ARG, ERR_CAPACITY, ERR_CUDA, ERR_NONFINITE, ERR_WORKSPACE, ERR_ORDER = 0
 FLAG_CAPTURE = 1
 FLAG_VERIFY_ORDER = 2
 FLAG_EQ5_ELECTRONS = 4
+FLAG_NO_FOLD = 8
+FLAG_FOLD_ALL = 16
 DBG_X, DBG_VX, DBG_VY, DBG_VZ, DBG_KEYS, DBG_OFFSETS, DBG_MASK, DBG_E32, DBG_RHO_S, DBG_TILE_W = range(10)
 _DBG_DTYPE = {DBG_X: np.float32, DBG_VX: np.float32, DBG_VY: np.float32, DBG_VZ: np.float32,
               DBG_KEYS: np.int32, DBG_OFFSETS: np.int32, DBG_MASK: np.uint8, DBG_E32: np.float32,

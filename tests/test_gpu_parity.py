@@ -20,7 +20,9 @@ def _mk(p):
     from paper_1104_3998_b200 import pic1d as G
     p = dict(p)
     hint = 0 if p.pop("no_hint", False) else (p["flags"] & G.FLAG_EQ5_ELECTRONS)
-    p["flags"] = G.FLAG_CAPTURE | G.FLAG_VERIFY_ORDER | hint
+    # where the MCC runs: folded into the scatter (forced for every species) or as a pass of its own
+    fold = G.FLAG_NO_FOLD if p.pop("no_fold", False) else G.FLAG_FOLD_ALL
+    p["flags"] = G.FLAG_CAPTURE | hint | fold
     parts = W.make_particles(p)
     o, g = O.Oracle(p), G.Pic1D(p)
     load(o, parts)
@@ -114,11 +116,13 @@ def test_electron_hint_only_changes_the_kernel_family():
         o.close(); g.close()
 
 
+@pytest.mark.parametrize("mcc", ["folded", "own_pass"])
 @pytest.mark.parametrize("name", list(CASES))
-def test_load_then_single_steps_from_identical_state(name):
+def test_load_then_single_steps_from_identical_state(name, mcc):
     """After the load and after each of a few steps (the oracle's E32 injected before every step so
-    both sides gather the identical field, R17) every discrete output is bit-exact."""
-    o, g, p = _mk(W.make_params(**CASES[name]))
+    both sides gather the identical field, R17) every discrete output is bit-exact -- with the
+    collisions folded into the scatter (default) and as a pass of their own (PIC1D_FLAG_NO_FOLD)."""
+    o, g, p = _mk(dict(W.make_params(**CASES[name]), no_fold=(mcc == "own_pass")))
     from oracle import oracle as O
     compare_state(o, g, p, check_keys=False)
     for n in range(4):
