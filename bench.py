@@ -161,6 +161,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fold", action="store_true",
                     help="run the collisions as a pass of their own (k_mcc) instead of folded into the scatter")
+    ap.add_argument("--no-overlap", action="store_true", help="collisions after the field solve, no side stream")
+    ap.add_argument("--no-graph", action="store_true", help="no CUDA graph replay in pic1d_step")
+    ap.add_argument("--mcc-gather", action="store_true", help="k_mcc without the bulk-copy staging of velocities")
     ap.add_argument("--fold-all", action="store_true", help="fold the collisions of every species into its scatter")
     ap.add_argument("--profile", action="store_true",
                     help="timed region only (no per-kernel pass, e2e or CPU baseline): the command ncu wraps")
@@ -175,6 +178,12 @@ def main():
         p["flags"] |= 8   # PIC1D_FLAG_NO_FOLD
     if args.fold_all:
         p["flags"] |= 16  # PIC1D_FLAG_FOLD_ALL
+    if args.mcc_gather:
+        p["flags"] |= 32  # PIC1D_FLAG_MCC_GATHER
+    if args.no_overlap:
+        p["flags"] |= 64  # PIC1D_FLAG_NO_OVERLAP
+    if args.no_graph:
+        p["flags"] |= 128  # PIC1D_FLAG_NO_GRAPH
 
     import torch
     import torch.distributed as dist

@@ -50,6 +50,13 @@ extern "C" {
  * its own after the field solve (k_mcc) otherwise. */
 #define PIC1D_FLAG_NO_FOLD 8u   /* never fold: every species gets the pass of its own */
 #define PIC1D_FLAG_FOLD_ALL 16u /* always fold */
+#define PIC1D_FLAG_MCC_GATHER 32u /* k_mcc fetches candidates' velocities with gathered loads even when most particles
+                                     are candidates (default then: bulk async copies of the tile into shared memory) */
+
+#define PIC1D_FLAG_NO_OVERLAP 64u /* run the collisions after the field solve on the caller's stream instead of beside
+                                    the deposit and the field solve on an internal side stream */
+#define PIC1D_FLAG_NO_GRAPH 128u  /* pic1d_step launches every kernel itself instead of replaying a captured CUDA graph
+                                     of two steps (a graph needs a capturable stream: not the legacy default stream) */
 
 typedef struct pic1d pic1d_t; /* opaque */
 
@@ -124,7 +131,8 @@ int pic1d_load_particles(pic1d_t* h, int species, int64_t n, const float* x, con
 /*
  * Enqueue n_steps full PIC/MCC cycles (Fig. 1, L35-41) on the stream.  Asynchronous: no host
  * synchronisation, no host round trip of rho or E (contrast L144).  Errors raised inside the
- * kernels are sticky and surface on the next synchronising call.
+ * kernels are sticky and surface on the next synchronising call.  Pairs of steps are replayed from a
+ * CUDA graph captured on first use (the step index and every particle count are device-resident).
  */
 int pic1d_step(pic1d_t* h, int n_steps);
 

@@ -72,6 +72,10 @@ struct pic1d {
     size_t smem_sort, smem_count[2], smem_scatter[2];
     void (*k_count[2])(SortArgs);
     void (*k_scatter[2][2])(SortArgs);  // [species][0 plain | 1 the step's, with the MCC folded in]
+    cudaStream_t side;              // collisions run here beside the deposit and the field solve
+    cudaEvent_t ev_fork, ev_join;
+    cudaGraphExec_t graph[2];       // two captured steps, per parity of the sort buffers at their start
+    int64_t launches_per_2steps;
     bool timing;
     std::vector<TimeMark> marks;
     std::vector<cudaEvent_t> ev_pool;
@@ -302,6 +306,8 @@ int occupancy_grid(pic1d* h, sort_kernel_t kernel, size_t smem) {
 // step's (with the species' MCC folded in, unless PIC1D_FLAG_NO_FOLD)
 void setup_launch(pic1d* h) {
     cudaFuncSetAttribute(k_field_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, FIELD_SMEM_MAX * (int)sizeof(double));
+    cudaFuncSetAttribute(k_mcc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
+    cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     h->WA = std::min((h->n_sc + 1 + 7) / 8 * 8, PIC1D_WA_MAX);
     h->smem_sort = (size_t)h->WA * sizeof(int);
     for (int s = 0; s < h->cfg.n_species; ++s) {
@@ -345,8 +351,6 @@ void enqueue_sort(pic1d* h, int s, int in_step, int shift = 0) {
     const int nb_null = fold ? (p.capacity / 32 + BINSCAN_NW * 32 - 1) / (BINSCAN_NW * 32) : 0;
     k_bin_scan<<<(a.n_sc + 31) / 32 + a.null_first + nb_null, BINSCAN_NW * 32, 0, h->stream>>>(a);
     mark(h, "bin_scan", s);
-    k_offsets_scan<<<1, 1024, 0, h->stream>>>(a);
-    mark(h, "offsets_scan", s);
     h->k_scatter[s][in_step]<<<gs, PIC1D_NT, h->smem_scatter[s], h->stream>>>(a);
     mark(h, "push_scatter", s);
     p.cur ^= 1;
@@ -366,24 +370,24 @@ void enqueue_begin(pic1d* h, int mode) {
     mark(h, "step_begin", -1);
 }
 
+// deposit of every species (one launch) + edge nodes, rho, Poisson and E (one block)
 void enqueue_grid(pic1d* h, int in_step) {
     const pic1d_config_t& c = h->cfg;
-    CombineArgs cb;
-    memset(&cb, 0, sizeof(cb));
+    DepositArgs d;
+    memset(&d, 0, sizeof(d));
+    FieldArgs f;
+    memset(&f, 0, sizeof(f));
+    CombineArgs& cb = f.cb;
     for (int s = 0; s < c.n_species; ++s) {
         SpeciesHost& p = h->sp[s];
-        DepositArgs d;
-        d.x = p.buf[p.cur][0]; d.offsets = p.offsets; d.part = p.part; d.side = p.side;
-        d.Nc = c.n_cells; d.n_sc = h->n_sc; d.G = h->G; d.inv_r = h->inv_r;
-        k_deposit<<<h->n_dep_blocks, PIC1D_NT, (h->G + 1) * (sizeof(ull) + 3 * sizeof(unsigned)), h->stream>>>(d);
-        mark(h, "deposit", s);
+        d.sp[s].x = p.buf[p.cur][0]; d.sp[s].offsets = p.offsets; d.sp[s].part = p.part; d.sp[s].side = p.side;
         cb.part[s] = p.part; cb.side[s] = p.side; cb.rho_s[s] = p.rho_s; cb.sign[s] = c.sp[s].charge_sign;
     }
+    d.Nc = c.n_cells; d.n_sc = h->n_sc; d.G = h->G; d.inv_r = h->inv_r;
+    k_deposit<<<dim3(h->n_dep_blocks, c.n_species), PIC1D_NT, (h->G + 1) * (sizeof(ull) + 3 * sizeof(unsigned)), h->stream>>>(d);
+    mark(h, "deposit", -1);
     cb.rho = h->rho; cb.n_species = c.n_species; cb.Nc = c.n_cells; cb.nodes = h->nodes; cb.G = h->G;
     cb.bc = c.bc; cb.background = c.background_rho;
-    k_rho_combine<<<(h->nodes + 255) / 256, 256, 0, h->stream>>>(cb);
-    mark(h, "rho_combine", -1);
-    FieldArgs f;
     f.rho = h->rho; f.phi = h->phi; f.E = h->E; f.S = h->S; f.Tt = h->Tt; f.E32 = h->E32;
     f.Nc = c.n_cells; f.nodes = h->nodes; f.bc = c.bc; f.V0 = c.V0_norm; f.omega_dt = c.omega_dt;
     f.st = h->st; f.in_step = in_step;
@@ -415,8 +419,10 @@ MccArgs mcc_args(pic1d* h, int s) {
     return m;
 }
 
-// the collisions that are not folded into a scatter, and the ionisation pairs
-void enqueue_mcc(pic1d* h) {
+// the collisions that are not folded into a scatter, and the ionisation pairs.  They depend on the sorted
+// particles only (not on rho or E, R3), so in a step they run on the side stream, beside the
+// deposit and the field solve.
+void enqueue_mcc(pic1d* h, cudaStream_t st) {
     const pic1d_config_t& c = h->cfg;
     for (int s = 0; s < c.n_species; ++s) {
         const int kind = c.sp[s].mcc_kind;
@@ -424,13 +430,16 @@ void enqueue_mcc(pic1d* h) {
         SpeciesHost& p = h->sp[s];
         MccArgs m = mcc_args(h, s);
         if (p.mcck == 0) {
-            const int grid = std::min(p.n_mcc_tiles, h->num_sms * 4);
-            if (kind == 1) k_mcc<1><<<grid, PIC1D_NT, 0, h->stream>>>(m);
-            else k_mcc<2><<<grid, PIC1D_NT, 0, h->stream>>>(m);
+            // dense candidates: the tile's velocities are streamed into shared memory by bulk async copies
+            const bool stage = c.sp[s].P0 > PIC1D_FOLD_P0_MAX && !(c.flags & PIC1D_FLAG_MCC_GATHER);
+            const int grid = std::min(p.n_mcc_tiles, h->num_sms * (stage ? 3 : 4));
+            const size_t sm = stage ? 3 * MCC_TILE * sizeof(float) : 0;
+            if (kind == 1) { if (stage) k_mcc<1, true><<<grid, PIC1D_NT, sm, st>>>(m); else k_mcc<1, false><<<grid, PIC1D_NT, 0, st>>>(m); }
+            else { if (stage) k_mcc<2, true><<<grid, PIC1D_NT, sm, st>>>(m); else k_mcc<2, false><<<grid, PIC1D_NT, 0, st>>>(m); }
             mark(h, "mcc", s);
         }
         if (kind == 1) {
-            k_mcc_births<<<h->num_sms, PIC1D_NT, 0, h->stream>>>(m);
+            k_mcc_births<<<h->num_sms * 4, PIC1D_NT, 0, st>>>(m);
             mark(h, "mcc_births", s);
         }
     }
@@ -454,8 +463,19 @@ void enqueue_step(pic1d* h) {
         }
     }
     enqueue_sort(h, 0, 1);
-    enqueue_grid(h, 1);
-    enqueue_mcc(h);
+    // fork: collisions + births on the side stream, deposit + field on the caller's; join at the end of the step
+    const bool overlap = h->side != nullptr && !h->timing && !(c.flags & PIC1D_FLAG_NO_OVERLAP);
+    if (overlap) {
+        cudaEventRecord(h->ev_fork, h->stream);
+        cudaStreamWaitEvent(h->side, h->ev_fork, 0);
+        enqueue_mcc(h, h->side);
+        cudaEventRecord(h->ev_join, h->side);
+        enqueue_grid(h, 1);
+        cudaStreamWaitEvent(h->stream, h->ev_join, 0);
+    } else {
+        enqueue_grid(h, 1);
+        enqueue_mcc(h, h->stream);
+    }
     h->step += 1u;
 }
 
@@ -514,6 +534,13 @@ int pic1d_create(const pic1d_config_t* cfg, void* workspace, size_t workspace_by
         return PIC1D_ERR_CUDA;
     }
     h->num_sms = prop.multiProcessorCount;
+    h->side = nullptr; h->graph[0] = h->graph[1] = nullptr;
+    if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        delete h;
+        return PIC1D_ERR_CUDA;
+    }
     setup_launch(h);
     h->last_err = cudaSuccess;
     // zero the bookkeeping (state, look-back descriptors); particle arrays need no initialisation
@@ -532,6 +559,8 @@ int pic1d_destroy(pic1d_t* h) {
     if (!h) return PIC1D_OK;
     cudaStreamSynchronize(h->stream);
     for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
+    for (int g = 0; g < 2; ++g) if (h->graph[g]) cudaGraphExecDestroy(h->graph[g]);
+    if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); cudaEventDestroy(h->ev_fork); cudaEventDestroy(h->ev_join); }
     delete h;
     return PIC1D_OK;
 }
@@ -595,7 +624,38 @@ int pic1d_load_particles(pic1d_t* h, int s, int64_t n, const float* x, const flo
 
 int pic1d_step(pic1d_t* h, int n_steps) {
     if (!h || n_steps < 0 || !h->ready) return PIC1D_ERR_ARG;
-    for (int k = 0; k < n_steps; ++k) enqueue_step(h);
+    int k = 0;
+    // Two consecutive steps (the sort buffers swap every step, so two steps restore the pointers) are captured
+    // once per buffer parity into a CUDA graph and replayed: every per-step quantity (step index, particle
+    // counts, tickets) lives in DevState on the device, no kernel argument changes from step to step.
+    if (!(h->cfg.flags & PIC1D_FLAG_NO_GRAPH)) {
+        while (n_steps - k >= 2) {
+            const int par = h->sp[0].cur;
+            if (!h->graph[par]) {
+                cudaGraph_t g = nullptr;
+                if (cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); break; }
+                const int64_t l0 = h->launches;
+                const uint32_t s0 = h->step;
+                enqueue_step(h);
+                enqueue_step(h);
+                h->launches_per_2steps = h->launches - l0;
+                h->launches = l0; h->step = s0;  // captured, not run
+                const cudaError_t e = cudaStreamEndCapture(h->stream, &g);
+                if (e != cudaSuccess || !g || cudaGraphInstantiate(&h->graph[par], g, 0) != cudaSuccess) {
+                    if (g) cudaGraphDestroy(g);
+                    h->graph[par] = nullptr;
+                    cudaGetLastError();
+                    break;
+                }
+                cudaGraphDestroy(g);
+            }
+            if (!ck(h, cudaGraphLaunch(h->graph[par], h->stream))) return PIC1D_ERR_CUDA;
+            h->launches += h->launches_per_2steps;
+            h->step += 2u;
+            k += 2;
+        }
+    }
+    for (; k < n_steps; ++k) enqueue_step(h);
     return ck(h, cudaGetLastError()) ? PIC1D_OK : PIC1D_ERR_CUDA;
 }
 

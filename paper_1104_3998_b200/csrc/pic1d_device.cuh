@@ -36,7 +36,7 @@ struct DevSpecies {
     int pool_used; // entries of the (tile x bin) count pool in use
     int ticket;    // dynamic tile counter of the MCC kernel
     int ticket2;   // dynamic tile counter of the scatter kernel
-    int pad_;
+    int scan_done; // bin blocks of k_bin_scan that have finished (the last one scans the histogram)
     ull absorbed_left, absorbed_right, injected, n_candidates, n_events[4], births, dropped, over_cap;
 };
 

@@ -4,12 +4,15 @@
 #pragma once
 #include "pic1d_device.cuh"
 
-struct DepositArgs {
+struct DepositSpecies {
     const float* x;      // sorted positions of the species
     const int* offsets;  // [n_sc + 1]
     double* part;        // [n_blocks * G]   nodes c0 .. c1-1 of each block (left-closed)
     double* side;        // [n_blocks]       right edge node c1 of each block (paper's side array, L138)
-    int Nc, n_sc, G;     // G grid cells per block (a multiple of the sort-cell size when r > 1)
+};
+struct DepositArgs {
+    DepositSpecies sp[2];  // blockIdx.y = species: one launch deposits every species
+    int Nc, n_sc, G;       // G grid cells per block (a multiple of the sort-cell size when r > 1)
     float inv_r;
 };
 
@@ -95,9 +98,12 @@ __device__ __forceinline__ void dep_row(bool valid, float xv, DepAcc& A, ull* s_
     }
 }
 
-__global__ void __launch_bounds__(PIC1D_NT) k_deposit(DepositArgs a) {
+__global__ void __launch_bounds__(PIC1D_NT) k_deposit(DepositArgs args) {
     extern __shared__ ull s_acc[];  // G + 1 nodes, then 3 x (G + 1) 32-bit limb counters
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    struct { const float* x; const int* offsets; double* part; double* side; int Nc, n_sc, G; float inv_r; } a;
+    a.x = args.sp[blockIdx.y].x; a.offsets = args.sp[blockIdx.y].offsets; a.part = args.sp[blockIdx.y].part;
+    a.side = args.sp[blockIdx.y].side; a.Nc = args.Nc; a.n_sc = args.n_sc; a.G = args.G; a.inv_r = args.inv_r;
     const int c0 = blockIdx.x * a.G, c1 = min(c0 + a.G, a.Nc);
     const int k0 = (int)__fmul_rn((float)c0, a.inv_r);
     const int k1 = c1 >= a.Nc ? a.n_sc : (int)__fmul_rn((float)c1, a.inv_r);
@@ -156,8 +162,8 @@ __global__ void __launch_bounds__(PIC1D_NT) k_deposit(DepositArgs a) {
     if (tid == 0) a.side[blockIdx.x] = node(c1 - c0);
 }
 
-// Follow-up kernel (L138): node j of species s = block part + the left neighbour's right-edge node;
-// net rho = background + sum_s sign_s rho_s.  One thread per node.
+// Follow-up step (L138; here the prologue of the field kernel, not a launch of its own): node j of species s =
+// block part + the left neighbour's right-edge node; net rho = background + sum_s sign_s rho_s.
 struct CombineArgs {
     const double* part[2];
     const double* side[2];
@@ -168,9 +174,7 @@ struct CombineArgs {
     double background;
 };
 
-__global__ void k_rho_combine(CombineArgs a) {
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= a.nodes) return;
+__device__ __forceinline__ void rho_combine_node(const CombineArgs& a, int j) {
     const int nb = (a.Nc + a.G - 1) / a.G;
     double r = a.background;
     for (int s = 0; s < a.n_species; ++s) {
@@ -193,6 +197,7 @@ __global__ void k_rho_combine(CombineArgs a) {
 // i.e. the Thomas recurrences (L142) summed in closed form, which turns the serial elimination into
 // two block-wide fp64 prefix sums.  E_j = (phi_{j-1} - phi_{j+1}) / 2 = -d_1 + (S_{j-1} + S_j) / 2.
 struct FieldArgs {
+    CombineArgs cb;  // the deposit's partial sums -> rho_s, rho (prologue)
     const double* rho;
     double *phi, *E, *S, *Tt;
     float* E32;
@@ -254,6 +259,8 @@ __device__ void block_inclusive_scan_d(F src, double* dst, int n) {
 
 __global__ void __launch_bounds__(1024) k_field(FieldArgs a) {
     const int N = a.Nc, tid = threadIdx.x;
+    for (int j = tid; j < a.nodes; j += blockDim.x) rho_combine_node(a.cb, j);
+    __syncthreads();
     double mean = 0.0;
     if (a.bc == 1) {
         double p = 0.0;
@@ -313,6 +320,8 @@ __global__ void __launch_bounds__(1024) k_field_smem(FieldArgs a) {
     const int N = a.Nc, tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
     const int seg = ((N + 1023) / 1024) * 32;  // elements per warp, a multiple of 32
     const double* rho = a.rho;
+    for (int j = tid; j < a.nodes; j += 1024) rho_combine_node(a.cb, j);
+    __syncthreads();
     double mean = 0.0;
     if (a.bc == 1) {
         double p = 0.0;

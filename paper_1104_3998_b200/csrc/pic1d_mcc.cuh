@@ -230,12 +230,42 @@ __device__ __forceinline__ int warp_append(bool flag, int* counter) {
     return base + __popc(bal & lanemask_lt());
 }
 
+// ---- bulk asynchronous copies (TMA engine, non-tensor form) + mbarrier ------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
 // ---- stand-alone pass over the sorted arrays -----------------------------------------------------------
 // KIND: 1 electron set, 2 ion charge exchange.  Persistent blocks take tiles of MCC_TILE sorted slots by
-// ticket; phases B / C fetch the candidates' velocities from global memory.
-template <int KIND>
-__global__ void __launch_bounds__(PIC1D_NT, 4) k_mcc(MccArgs a) {
+// ticket.  STAGE (species most of whose particles are candidates): the tile's vx, vy, vz are streamed into
+// shared memory by three bulk asynchronous copies (cp.async.bulk, completion on an mbarrier) that fly while
+// phase A computes the null tests, so phases B / C never wait for a gathered global load; otherwise phases
+// B / C fetch the few candidates' velocities from global memory.
+template <int KIND, bool STAGE>
+__global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
     constexpr int TILE = MCC_TILE;
+    extern __shared__ __align__(128) float s_v[];  // STAGE: [3][TILE]
+    __shared__ unsigned long long s_bar;
     __shared__ int s_tile;
     __shared__ int s_n[2];                   // candidates, real collisions
     __shared__ unsigned short s_cand[TILE];  // slot - tile base
@@ -249,8 +279,19 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_mcc(MccArgs a) {
     const uint32_t step = st->step;
     const uint32_t str_null = STREAM_NULL + (uint32_t)m.s, str_coll = STREAM_COLL + (uint32_t)m.s;
     MccCount cnt = {0u, 0u, 0u};
+    unsigned parity = 0;
+    if (STAGE && tid == 0) mbar_init(&s_bar, 1);
     while (true) {
-        if (tid == 0) { s_tile = atomicAdd(&sp.ticket, 1); s_n[0] = 0; s_n[1] = 0; }
+        if (tid == 0) {
+            const int t = atomicAdd(&sp.ticket, 1);
+            s_tile = t; s_n[0] = 0; s_n[1] = 0;
+            if (STAGE && t < n_act) {  // the arrays hold capacity slots, a multiple of TILE: a whole tile is always in bounds
+                mbar_expect_tx(&s_bar, 3u * TILE * sizeof(float));
+                bulk_g2s(s_v, a.vx + (size_t)t * TILE, TILE * sizeof(float), &s_bar);
+                bulk_g2s(s_v + TILE, a.vy + (size_t)t * TILE, TILE * sizeof(float), &s_bar);
+                bulk_g2s(s_v + 2 * TILE, a.vz + (size_t)t * TILE, TILE * sizeof(float), &s_bar);
+            }
+        }
         __syncthreads();
         const int tile = s_tile;
         if (tile >= n_act) break;
@@ -293,6 +334,7 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_mcc(MccArgs a) {
             }
         }
         __syncthreads();
+        if (STAGE) { mbar_wait(&s_bar, parity); parity ^= 1u; }
         // ---- phase B: process selection, one thread per candidate ----------------------------------
         const int n_cand = s_n[0];
         for (int j0 = 0; j0 < n_cand; j0 += PIC1D_NT) {
@@ -302,7 +344,8 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_mcc(MccArgs a) {
             if (j < n_cand) {
                 rel = s_cand[j];
                 const int i = tbase + rel;
-                const float vx = a.vx[i], vy = a.vy[i], vz = a.vz[i];
+                const float vx = STAGE ? s_v[rel] : a.vx[i], vy = STAGE ? s_v[TILE + rel] : a.vy[i],
+                            vz = STAGE ? s_v[2 * TILE + rel] : a.vz[i];
                 uint32_t b0[4];
                 philox4x32_10((uint32_t)i, step, str_coll, 0u, m.k0, m.k1, b0);
                 bool over;
@@ -325,7 +368,7 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_mcc(MccArgs a) {
             philox4x32_10((uint32_t)i, step, str_coll, 0u, m.k0, m.k1, b0);
             float vx, vy, vz;
             if (KIND == 1) {
-                vx = a.vx[i]; vy = a.vy[i]; vz = a.vz[i];
+                vx = STAGE ? s_v[rel] : a.vx[i]; vy = STAGE ? s_v[TILE + rel] : a.vy[i]; vz = STAGE ? s_v[2 * TILE + rel] : a.vz[i];
                 const float gp = mcc_electron_kinematics(m, e, vx, vy, vz, u01(b0[1]), u01(b0[2]));
                 if (e == 3) mcc_record_ionisation(m, (unsigned)i, gp);
             } else {

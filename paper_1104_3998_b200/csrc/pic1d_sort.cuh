@@ -204,7 +204,7 @@ __device__ int block_exclusive_scan(const int* src, int* dst, int n) {
     for (int i = b + lane; i < e; i += 32 * 8) {
         int v[8];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) v[u] = i + u * 32 < e ? src[i + u * 32] : 0;
+        for (int u = 0; u < 8; ++u) v[u] = i + u * 32 < e ? __ldcg(src + i + u * 32) : 0;
 #pragma unroll
         for (int u = 0; u < 8; ++u) tot += v[u];
     }
@@ -228,7 +228,7 @@ __device__ int block_exclusive_scan(const int* src, int* dst, int n) {
     for (int i0 = b; i0 < e; i0 += 32 * 4) {
         int v[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) v[u] = i0 + u * 32 + lane < e ? src[i0 + u * 32 + lane] : 0;
+        for (int u = 0; u < 4; ++u) v[u] = i0 + u * 32 + lane < e ? __ldcg(src + i0 + u * 32 + lane) : 0;
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             if (SPARSE && !__any_sync(0xffffffffu, v[u] != 0)) continue;
@@ -251,6 +251,27 @@ __device__ int block_exclusive_scan(const int* src, int* dst, int n) {
 // over the warps.  Pass 1 sums each warp's share, a shared-memory prefix orders the warps, pass 2
 // rewrites pool[tile_off[t] + k - tile_lo[t]] as the number of particles of tiles < t with key k
 // (exclusive prefix over tiles); hist[k] gets the total.  Row segments of the pool are read coalesced.
+// The bin block that finishes last turns the histogram into offsets[k] = #{key < k} and closes the sort's
+// counts (n_live = n_sorted = survivors): the former k_offsets_scan, saved as a launch.
+__device__ void bin_scan_finish(const SortArgs& a) {
+    __shared__ int s_last;
+    DevSpecies& sp = a.st->sp[a.s];
+    __syncthreads();  // this block's hist entries are written
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_last = atomicAdd(&sp.scan_done, 1) == (a.n_sc + 31) / 32 - 1;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    const int total = block_exclusive_scan<false>(a.hist, a.offsets, a.n_sc);
+    if (threadIdx.x == 0) {
+        a.offsets[a.n_sc] = total;
+        sp.n_live = total;
+        sp.n_sorted = total;
+    }
+}
+
 #define BINSCAN_NW 32
 #define BINSCAN_LIST 4096
 #define BINSCAN_DESC 2048  // tile descriptors a block can keep in shared memory
@@ -363,6 +384,7 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
             for (int b = 0; b < B; ++b) if (p[b]) { __stcg(p[b], run); run += c[b]; }
         }
         if (wp == 0 && k < a.n_sc) a.hist[k] = total;
+        bin_scan_finish(a);
         return;
     }
     int sum = 0;
@@ -414,17 +436,7 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
         for (int b = 0; b < B; ++b) if (p[b]) { __stcg(p[b], run); run += c[b]; }
     }
     if (wp == 0 && k < a.n_sc) a.hist[k] = total;
-}
-
-// offsets[k] = #{key < k}; n_live = n_sorted = survivors.
-__global__ void __launch_bounds__(1024) k_offsets_scan(SortArgs a) {
-    DevSpecies& sp = a.st->sp[a.s];
-    const int total = block_exclusive_scan<false>(a.hist, a.offsets, a.n_sc);
-    if (threadIdx.x == 0) {
-        a.offsets[a.n_sc] = total;
-        sp.n_live = total;
-        sp.n_sorted = total;
-    }
+    bin_scan_finish(a);
 }
 
 // ---- pass 2 -----------------------------------------------------------------------------------
@@ -734,6 +746,7 @@ __global__ void k_step_begin(BeginArgs b) {
             sp.pool_used = 0;
             sp.ticket = 0;
             sp.ticket2 = 0;
+            sp.scan_done = 0;
         }
         st->n_abs = 0;
         if (b.mode) { st->step = st->step_next; st->step_next = st->step + 1u; }

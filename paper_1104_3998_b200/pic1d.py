@@ -18,6 +18,9 @@ FLAG_VERIFY_ORDER = 2
 FLAG_EQ5_ELECTRONS = 4
 FLAG_NO_FOLD = 8
 FLAG_FOLD_ALL = 16
+FLAG_MCC_GATHER = 32
+FLAG_NO_OVERLAP = 64
+FLAG_NO_GRAPH = 128
 DBG_X, DBG_VX, DBG_VY, DBG_VZ, DBG_KEYS, DBG_OFFSETS, DBG_MASK, DBG_E32, DBG_RHO_S, DBG_TILE_W = range(10)
 _DBG_DTYPE = {DBG_X: np.float32, DBG_VX: np.float32, DBG_VY: np.float32, DBG_VZ: np.float32,
               DBG_KEYS: np.int32, DBG_OFFSETS: np.int32, DBG_MASK: np.uint8, DBG_E32: np.float32,
@@ -126,7 +129,8 @@ class Pic1D:
             raise Pic1DError("pic1d_workspace_bytes", rc)
         self.workspace_bytes = nbytes.value
         self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
-        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        # a stream of its own: the legacy default stream cannot be captured into a CUDA graph
+        self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
         self.h = C.c_void_p()
         rc = self.lib.pic1d_create(C.byref(self.cfg), C.c_void_p(self.workspace.data_ptr()), nbytes,
                                    C.c_void_p(self.stream.cuda_stream), C.byref(self.h))
