@@ -191,6 +191,14 @@ int pic1d_debug_get(pic1d_t* h, int what, int species, void* dst, size_t bytes);
  * identical state, R17).  E32: HOST, n_nodes floats. */
 int pic1d_debug_set_E32(pic1d_t* h, const float* E32, int n_nodes);
 
+/* Overwrite the live particles of a species IN PLACE, keeping their order: slots [0, n_sorted) are taken as
+ * the sorted part, [n_sorted, n) as the birth tail; nothing is sorted, deposited or solved.  step >= 0 also sets
+ * the index of the next step.  The parity harness uses it to start EVERY compared step from the oracle's exact
+ * state (velocities of collided particles otherwise differ in the last bits: libm vs CUDA sin / cos / log), so
+ * that the single-step bars of north_star (x bit-exact, rho 1e-9) apply to every step.  HOST arrays, copied. */
+int pic1d_debug_set_state(pic1d_t* h, int species, int64_t n, int64_t n_sorted, const float* x, const float* vx,
+                          const float* vy, const float* vz, int64_t step);
+
 #ifdef __cplusplus
 }
 #endif

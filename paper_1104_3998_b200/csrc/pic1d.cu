@@ -775,6 +775,26 @@ int pic1d_debug_get(pic1d_t* h, int what, int s, void* dst, size_t bytes) {
     return ck(h, cudaStreamSynchronize(h->stream)) ? PIC1D_OK : PIC1D_ERR_CUDA;
 }
 
+__global__ void k_debug_set_counts(DevState* st, int s, int n_live, int n_sorted, int set_step, unsigned step) {
+    st->sp[s].n_live = n_live;
+    st->sp[s].n_sorted = n_sorted;
+    if (set_step) st->step_next = step;
+}
+
+int pic1d_debug_set_state(pic1d_t* h, int s, int64_t n, int64_t n_sorted, const float* x, const float* vx,
+                          const float* vy, const float* vz, int64_t step) {
+    if (!h || s < 0 || s >= h->cfg.n_species || !h->ready || n < 0 || n_sorted < 0 || n_sorted > n) return PIC1D_ERR_ARG;
+    SpeciesHost& p = h->sp[s];
+    if (n > p.capacity) return PIC1D_ERR_CAPACITY;
+    const float* src[4] = {x, vx, vy, vz};
+    for (int k = 0; k < 4 && n > 0; ++k)
+        if (!src[k] || !ck(h, cudaMemcpyAsync(p.buf[p.cur][k], src[k], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, h->stream)))
+            return PIC1D_ERR_CUDA;
+    k_debug_set_counts<<<1, 1, 0, h->stream>>>(h->st, s, (int)n, (int)n_sorted, step >= 0 ? 1 : 0, (unsigned)(step >= 0 ? step : 0));
+    if (step >= 0) h->step = (uint32_t)step;
+    return ck(h, cudaStreamSynchronize(h->stream)) ? PIC1D_OK : PIC1D_ERR_CUDA;
+}
+
 int pic1d_debug_set_E32(pic1d_t* h, const float* E32, int n_nodes) {
     if (!h || !E32 || n_nodes != h->nodes) return PIC1D_ERR_ARG;
     if (!ck(h, cudaMemcpyAsync(h->E32, E32, sizeof(float) * n_nodes, cudaMemcpyHostToDevice, h->stream))) return PIC1D_ERR_CUDA;

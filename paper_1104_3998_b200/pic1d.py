@@ -29,7 +29,8 @@ _DBG_DTYPE = {DBG_X: np.float32, DBG_VX: np.float32, DBG_VY: np.float32, DBG_VZ:
 EXPORTS = ["pic1d_workspace_bytes", "pic1d_create", "pic1d_load_particles", "pic1d_step",
            "pic1d_get_rho_phi_E", "pic1d_moments", "pic1d_destroy", "pic1d_n_nodes",
            "pic1d_n_sort_cells", "pic1d_step_index", "pic1d_last_cuda_error", "pic1d_launch_count",
-           "pic1d_step_timed", "pic1d_debug_count", "pic1d_debug_get", "pic1d_debug_set_E32"]
+           "pic1d_step_timed", "pic1d_debug_count", "pic1d_debug_get", "pic1d_debug_set_E32",
+           "pic1d_debug_set_state"]
 
 
 class SpeciesConfig(C.Structure):
@@ -226,6 +227,14 @@ class Pic1D:
         rc = self.lib.pic1d_debug_set_E32(self.h, _ptr(a), C.c_int(a.shape[0]))
         if rc:
             self._err("pic1d_debug_set_E32", rc)
+
+    def set_state(self, s, n_sorted, x, vx, vy, vz, step=-1):
+        """debug: overwrite the live particles of species s in place (order kept); see pic1d_debug_set_state"""
+        arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in (x, vx, vy, vz)]
+        rc = self.lib.pic1d_debug_set_state(self.h, C.c_int(s), C.c_int64(arrs[0].shape[0]), C.c_int64(n_sorted),
+                                            *[_ptr(a) for a in arrs], C.c_int64(step))
+        if rc:
+            self._err("pic1d_debug_set_state", rc)
 
     @property
     def step_index(self):
