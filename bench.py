@@ -79,18 +79,22 @@ class ClockSampler(threading.Thread):
 
 
 # ---------------------------------------------------------------------------------------------
-def run_oracle_sample(p_full, steps, warmup):
-    """The oracle as it stands, one thread, on a bounded sample of the workload: same grid, same
-    constants, ppc reduced so that the run takes seconds."""
+def run_oracle_sample(p_full, steps, warmup, full_size=True):
+    """The oracle as it stands, one thread, on the workload itself (config 4 at its full size,
+    >= 3 timed steps, ~5 s each) -- or, full_size=False, on the same grid with ppc cut to 100."""
     from oracle import oracle as O
-    ppc = max(8, min(p_full["ppc"], 100))
-    p = W.make_params(p_full["cfg_id"], n_cells=p_full["n_cells"], ppc=ppc, sort_ratio=p_full["sort_ratio"],
-                      courant=p_full["courant"])
+    if full_size:
+        p = dict(p_full)
+    else:
+        p = W.make_params(p_full["cfg_id"], n_cells=p_full["n_cells"], ppc=max(8, min(p_full["ppc"], 100)),
+                          sort_ratio=p_full["sort_ratio"], courant=p_full["courant"])
     parts = W.make_particles(p)
     o = O.Oracle(p)
     for s, a in enumerate(parts):
         o.load_particles(s, *a)
-    o.step(warmup)
+    del parts
+    if warmup:
+        o.step(warmup)
     n0 = sum(o.moments(s)["count"] for s in range(p["n_species"]))
     t0 = time.perf_counter()
     o.step(steps)
@@ -98,9 +102,9 @@ def run_oracle_sample(p_full, steps, warmup):
     n1 = sum(o.moments(s)["count"] for s in range(p["n_species"]))
     o.close()
     value = 0.5 * (n0 + n1) * steps / dt
-    sample = "%s at ppc=%d (%d particles; the timed workload has ppc=%d), %d steps after %d warm-up" % (
-        p["name"], ppc, n0, p_full["ppc"], steps, warmup)
-    return value, dt / steps * 1e3, sample
+    sample = "%s at ppc=%d (%d particles; the timed GPU workload has ppc=%d), steps %d..%d of the run, oracle single-threaded" % (
+        p["name"], p["ppc"], n0, p_full["ppc"], warmup, warmup + steps)
+    return value, dt / steps * 1e3, sample, p["ppc"] == p_full["ppc"]
 
 
 def cpu_model():
@@ -114,36 +118,64 @@ def cpu_model():
 
 
 def reference_arm(args, p):
+    """--impl reference: the oracle on the host cores, same config / metric / unit; every "step" is a full-size
+    oracle step, their number capped so that the run ends within a few minutes (said in the line)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    steps = max(1, min(args.steps, 10))
-    value, ms, sample = run_oracle_sample(p, steps, min(args.warmup, 2))
+    steps = max(1, min(args.steps, 6 if p["n_per_species"] > 10_000_000 else 50))
+    value, ms, sample, same = run_oracle_sample(p, steps, min(args.warmup, 1))
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(p), "timed": sample},
+        "config": {"workload": workload_name(p), "timed": sample, "timed_steps": steps},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
-                         "host_cpu": cpu_model(), "nproc": os.cpu_count()},
+                         "same_config": same, "host_cpu": cpu_model(), "nproc": os.cpu_count()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
 
 # ---------------------------------------------------------------------------------------------
-def algorithmic_bytes(name, n_src, n_out, n_sorted, cand_frac, coll_frac):
-    """SURVEY 8(d)-D4 / DESIGN.md: bytes the method must move, per launch"""
+def mcc_bytes_per_particle(cand_frac, coll_frac):
+    """12 B of velocity read for every 32-byte sector that holds a candidate, 12 B written per sector with a collision"""
+    return 12.0 * (1.0 - (1.0 - cand_frac) ** 8), 12.0 * (1.0 - (1.0 - coll_frac) ** 8)
+
+
+def algorithmic_bytes(name, n_src, n_out, cand_frac, coll_frac, folded):
+    """SURVEY 8(d)-D4 / DESIGN.md section 6: bytes the method must move, per launch of the pipeline AS BUILT"""
     if name == "push_count":
         return 8.0 * n_src                       # read x, vx
     if name == "push_scatter":
-        return 16.0 * n_src + 16.0 * n_out       # read 4 arrays, write 4 arrays
+        return 16.0 * n_src + 16.0 * n_out       # read 4 arrays, write 4 arrays (folded MCC: nothing more)
+    if name == "bin_scan" and folded:
+        return n_src / 8.0                       # null-test bit mask written (read again by the scatter: L2)
     if name == "deposit":
-        return 4.0 * n_sorted                    # read sorted x
+        return 4.0 * n_out                       # read sorted x
     if name == "mcc":
-        rd = 12.0 * (1.0 - (1.0 - cand_frac) ** 8)
-        wr = 12.0 * (1.0 - (1.0 - coll_frac) ** 8)
-        return (rd + wr) * n_sorted
+        rd, wr = mcc_bytes_per_particle(cand_frac, coll_frac)
+        return (rd + wr) * n_out
     return 0.0
+
+
+def canonical_bytes(n_src, n_out, cand_frac, coll_frac):
+    """SURVEY 8(d)-D4's canonical store-between pipeline: push 16 + histogram 0 + scatter 32 + deposit 4 = 52 B
+    per particle-step, + MCC as its own pass"""
+    rd, wr = mcc_bytes_per_particle(cand_frac, coll_frac)
+    return 16.0 * n_src + 16.0 * n_src + 16.0 * n_out + 4.0 * n_out + (rd + wr) * n_out
+
+
+def read_traffic(kernel):
+    """profiles/r2_traffic.txt: `kernel[s=..] dram_bytes n_src n_out` of ONE ncu --set full capture (per launch),
+    with the live counts of the captured launch, so the ratio to the algorithmic bytes is like for like"""
+    tf = os.path.join(ROOT, "profiles", "r2_traffic.txt")
+    if not os.path.exists(tf):
+        return None
+    for line in open(tf):
+        w = line.split()
+        if len(w) >= 4 and w[0] == kernel:
+            return {"dram_bytes": float(w[1]), "n_src": float(w[2]), "n_out": float(w[3])}
+    return None
 
 
 def main():
@@ -159,6 +191,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-200", action="store_true", help="skip the 200-step average of config 4")
     ap.add_argument("--no-fold", action="store_true",
                     help="run the collisions as a pass of their own (k_mcc) instead of folded into the scatter")
     ap.add_argument("--no-overlap", action="store_true", help="collisions after the field solve, no side stream")
@@ -262,38 +295,77 @@ def main():
     peak, peak_src = measured_peak()
     kern = []
     dom = None
-    for (name, s), (tms, cnt) in sorted(agg.items(), key=lambda kv: -kv[1][0]):
+    folded = {s_: (p["species"][s_]["P0"] <= 0.25 or args.fold_all) and not args.no_fold and p["species"][s_]["mcc_kind"] != 0
+              for s_ in range(ns)}
+    stat = {}
+    for s_ in range(ns):
+        n_in = 0.5 * (mk0[s_]["count"] + mk1[s_]["count"])
+        n_out = 0.5 * (mk0[s_]["n_sorted"] + mk1[s_]["n_sorted"])
+        cand = (mk1[s_]["n_candidates"] - mk0[s_]["n_candidates"]) / max(ksteps * n_out, 1)
+        coll = sum(mk1[s_]["n_events"][k] - mk0[s_]["n_events"][k] for k in range(1, 4)) / max(ksteps * n_out, 1)
+        stat[s_] = (n_in, n_out, cand, coll)
+    for (name, s_), (tms, cnt) in sorted(agg.items(), key=lambda kv: -kv[1][0]):
         avg = tms / cnt
-        row = {"kernel": name, "species": s, "ms": avg, "share": tms / ksteps / step_ms_timed}
-        if s >= 0:
-            n_in = 0.5 * (mk0[s]["count"] + mk1[s]["count"])
-            n_out = 0.5 * (mk0[s]["n_sorted"] + mk1[s]["n_sorted"])
-            d = {k: mk1[s][k] - mk0[s][k] for k in ("n_candidates",)}
-            dev_ev = [mk1[s]["n_events"][k] - mk0[s]["n_events"][k] for k in range(4)]
-            cand = d["n_candidates"] / max(ksteps * n_out, 1)
-            coll = sum(dev_ev[1:]) / max(ksteps * n_out, 1)
-            b = algorithmic_bytes(name, n_in, n_out, n_out, cand, coll)
-            if b > 0:
-                row["alg_bytes"] = b
-                row["alg_GBps"] = b / (avg * 1e-3) / 1e9
-                row["frac_of_peak"] = row["alg_GBps"] / peak
+        row = {"kernel": name, "species": s_, "ms": avg, "share": tms / ksteps / step_ms_timed}
+        if s_ >= 0:
+            n_in, n_out, cand, coll = stat[s_]
+            bts = algorithmic_bytes(name, n_in, n_out, cand, coll, folded[s_])
+        elif name == "deposit":
+            bts = sum(algorithmic_bytes(name, stat[q][0], stat[q][1], 0, 0, False) for q in range(ns))
+        else:
+            bts = 0.0
+        if bts > 0:
+            row["alg_bytes"] = bts
+            row["alg_GBps"] = bts / (avg * 1e-3) / 1e9
+            row["frac_of_peak"] = row["alg_GBps"] / peak
         kern.append(row)
         if dom is None and "alg_GBps" in row:
             dom = row
+    step_s = ms_max / args.steps * 1e-3
     step_bytes = sum(r.get("alg_bytes", 0.0) for r in kern)
-    roofline = {"bound": "hbm", "kernel": "%s[s=%d]" % (dom["kernel"], dom["species"]),
+    canon = sum(canonical_bytes(*stat[q]) for q in range(ns))
+    n_live = sum(stat[q][0] for q in range(ns))
+    dom_name = "%s[s=%d]" % (dom["kernel"], dom["species"])
+    roofline = {"bound": "hbm", "kernel": dom_name,
                 "achieved": dom["alg_GBps"], "peak": peak, "unit": "GB/s", "frac": dom["alg_GBps"] / peak,
                 "traffic": None, "peak_source": peak_src, "alg_bytes_per_launch": dom["alg_bytes"],
-                "kernel_ms": dom["ms"],
-                "step": {"alg_bytes": step_bytes, "achieved": step_bytes / (ms_max / args.steps * 1e-3) / 1e9,
-                         "frac": step_bytes / (ms_max / args.steps * 1e-3) / 1e9 / peak,
-                         "frac_of_8TBps": step_bytes / (ms_max / args.steps * 1e-3) / 1e9 / 8000.0}}
-    tf = os.path.join(ROOT, "profiles", "traffic.txt")
-    if os.path.exists(tf):
-        for line in open(tf):
-            w = line.split()
-            if len(w) >= 2 and w[0] == roofline["kernel"]:
-                roofline["traffic"] = float(w[1])
+                "kernel_ms": dom["ms"], "particles_per_launch": stat[dom["species"]][0],
+                "step": {"as_built": {"bytes_per_particle": step_bytes / n_live, "alg_bytes": step_bytes,
+                                      "achieved": step_bytes / step_s / 1e9, "frac": step_bytes / step_s / 1e9 / peak,
+                                      "frac_of_8TBps": step_bytes / step_s / 1e9 / 8000.0,
+                                      "pipeline": "count 8 + scatter 32 + deposit 4 = 44 B + MCC (own pass: sectors touched; folded: 1/8 B bit mask)"},
+                         "canonical_52B": {"bytes_per_particle": canon / n_live, "alg_bytes": canon,
+                                           "achieved": canon / step_s / 1e9, "frac": canon / step_s / 1e9 / peak,
+                                           "frac_of_8TBps": canon / step_s / 1e9 / 8000.0,
+                                           "pipeline": "SURVEY 8(d)-D4: push 16 + scatter 32 + deposit 4 = 52 B + MCC pass"}}}
+    tr = read_traffic(dom_name)
+    if tr:   # one ncu --set full capture; its own particle counts make the ratio like for like
+        roofline["traffic"] = tr["dram_bytes"]
+        roofline["traffic_state"] = {"n_src": tr["n_src"], "n_out": tr["n_out"], "source": "profiles/r2_traffic.txt"}
+        roofline["traffic_alg_ratio"] = tr["dram_bytes"] / max(
+            algorithmic_bytes(dom["kernel"], tr["n_src"], tr["n_out"], 0, 0, False), 1.0)
+
+    # the workload is not stationary (electrons are lost to the walls and heated, ions multiply): config 4 is
+    # defined as 200 steps, so the average over its whole run is reported beside the timed window
+    run200 = None
+    if args.config == 4 and not args.no_200 and world == 1:
+        for s_, sp in enumerate(pinned):
+            sim.load_particles(s_, *[t_.numpy() for t_ in sp])
+        tot_ms, tot_ps, chunk = 0.0, 0.0, 10
+        c0 = sum(m["count"] for m in live())
+        for _ in range(200 // chunk):
+            barrier()
+            e0.record(sim.stream)
+            sim.step(chunk)
+            e1.record(sim.stream)
+            barrier()
+            tot_ms += e0.elapsed_time(e1)
+            c1 = sum(m["count"] for m in live())
+            tot_ps += 0.5 * (c0 + c1) * chunk
+            c0 = c1
+        run200 = {"value_200": tot_ps / (tot_ms * 1e-3), "ms_per_step_200": tot_ms / 200.0, "unit": UNIT,
+                  "window": "steps 0..200 after a fresh load (config 4's own run), timed in 20 chunks of 10 steps",
+                  "particles_first_last": [2 * p["n_per_species"], c1]}
 
     # end to end through the public API with HOST buffers: every step re-loads the particles from
     # pinned host memory (H2D), advances one step, and reads rho/phi/E back (D2H)
@@ -320,8 +392,10 @@ def main():
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, cms, sample = run_oracle_sample(p, 5, 1)
-        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+        del pinned, parts
+        sim.close()
+        v, cms, sample, same = run_oracle_sample(p, 3, 0)     # >= 3 timed steps at full size
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "same_config": same,
                "ms_per_step": cms, "host_cpu": cpu_model(), "nproc": os.cpu_count()}
 
     if rank == 0:
@@ -330,15 +404,19 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(p), "particles_per_gpu": n_mean,
+                       "window": "steps %d..%d after the load (the workload is not stationary: see run_200)" % (
+                           args.warmup, args.warmup + args.steps),
                        "l2": "inputs larger than L2 (%.2f GB of particle state per GPU)" % (n_mean * 16 / 1e9),
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "capture_masks": False,
+                       "mcc": {("electrons", "ions")[q]: ("folded into the scatter" if folded[q] else "own pass (k_mcc)") for q in range(ns)},
+                       "cuda_graph": not args.no_graph, "mcc_beside_field_solve": not args.no_overlap,
                        "sort": ("electrons and ions: warp tiles of 256 slots" if p["flags"] & 4 else
                                 "electrons: block tiles of 2048 slots (staged scatter); ions: warp tiles of 256 slots")},
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": args.e2e_steps, "note": "load_particles(host) + step(1) + get_rho_phi_E(host) per step"},
-            "roofline": roofline, "cpu_baseline": cpu,
+            "roofline": roofline, "cpu_baseline": cpu, "run_200": run200,
             "kernels": kern, "ms_per_step_with_kernel_events": step_ms_timed}))
     if world > 1:
         dist.destroy_process_group()

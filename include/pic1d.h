@@ -42,9 +42,20 @@ extern "C" {
                                       groups in slot order, so there is no hardware ordering left to verify */
 #define PIC1D_FLAG_EQ5_ELECTRONS 4u /* hint: the electrons obey Eq. 5 (L162: they move less than about one sort
                                        cell per step), so they take the barrier-free warp-tile sort like the
-                                       ions.  Only a performance hint: both sort families are correct for any
-                                       displacement. */
-
+                                       ions.  A performance hint within the displacement limits below. */
+/*
+ * Displacement limits of the fine sort.  The sort keeps, per tile of consecutive source slots, one counter per
+ * sort cell of the tile's key WINDOW (lowest to highest key after the push).  Each tile owns a fixed row of
+ * counters -- 32 sort cells for the warp-tile family (256 slots per tile: ions, electrons with the Eq. 5 hint),
+ * min(N_sc, 4096) for the block-tile family (2048 or 1024 slots per tile: electrons) -- and wider windows draw
+ * from an overflow region of max(4 Mi, capacity) counters per species.  Both families are exact for ANY
+ * displacement as long as that region lasts: the windows beyond the fixed rows may sum to `capacity` sort cells,
+ * i.e. on average 256 + 32 sort cells per warp tile (thermal displacement up to about 48 sort cells per step) and
+ * 2048 + 4096 per block tile.  If it runs out, the tiles that got no counters are LOST: their particles are
+ * counted in pic1d_moments_t.dropped and the sticky error PIC1D_ERR_WORKSPACE is raised -- the run is invalid
+ * from that step on (clear the Eq. 5 hint, or raise the species' capacity).  An unsorted load never needs the
+ * overflow region (it is sorted by leading key bits first).
+ */
 /* Where the Monte-Carlo collisions of a species run (same results either way).  Default: folded into the
  * scatter of its fine sort when its null-collision probability P0 <= 0.25 (sparse candidates), as a pass of
  * its own after the field solve (k_mcc) otherwise. */

@@ -172,7 +172,7 @@ size_t layout(pic1d* h, char* base) {
         p.grp_lo = carve<int>(base, off, p.n_groups_max);
         p.grp_hi = carve<int>(base, off, p.n_groups_max);
         // count pool: one fixed row of pool_stride bins per tile + an overflow region for wider windows
-        const int64_t over = std::max<int64_t>(4 << 20, p.capacity / 4);
+        const int64_t over = std::max<int64_t>(4 << 20, p.capacity);  // see pic1d.h, "Displacement limits"
         int64_t stride = p.warp_tiles ? PIC1D_PSW : std::min<int64_t>((h->n_sc + 3) / 4 * 4, 4096);
         if (!p.warp_tiles) stride = std::max<int64_t>(4, std::min<int64_t>(stride, (((1ll << 31) - 1 - over) / p.n_tiles_max) / 4 * 4));
         p.pool_stride = (int)stride;
@@ -586,7 +586,12 @@ int pic1d_load_particles(pic1d_t* h, int s, int64_t n, const float* x, const flo
     k_validate<<<(int)std::min<int64_t>(1024, n / 256 + 1), 256, 0, h->stream>>>(p.buf[0][0], (int)n, (float)h->cfg.n_cells, h->st);
     h->launches += 2;
     h->loaded_mask |= 1 << s;
-    if (h->loaded_mask != (1 << h->cfg.n_species) - 1) return ck(h, cudaGetLastError()) ? PIC1D_OK : PIC1D_ERR_CUDA;
+    if (h->loaded_mask != (1 << h->cfg.n_species) - 1) {
+        if (!ck(h, cudaGetLastError())) return PIC1D_ERR_CUDA;
+        // host arrays are "copied; the caller keeps ownership": they may be reused or freed as soon as we return
+        if (!on_device && !ck(h, cudaStreamSynchronize(h->stream))) return PIC1D_ERR_CUDA;
+        return PIC1D_OK;
+    }
     // last species in: fine-sort, deposit and solve so that rho / phi / E are valid for step 0
     h->loaded_mask = 0;
     h->step = 0;
