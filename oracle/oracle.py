@@ -15,9 +15,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "pic1d_oracle.c")
 _LIB = os.path.join(_HERE, "libpic1d_oracle.so")
 
-X, VX, VY, VZ, KEYS, OFFSETS, MASK, E32, RHO_S = range(9)
+X, VX, VY, VZ, KEYS, OFFSETS, MASK, E32, RHO_S, PARTNER = range(10)
 _DTYPES = {X: np.float32, VX: np.float32, VY: np.float32, VZ: np.float32, KEYS: np.int32,
-           OFFSETS: np.int32, MASK: np.uint8, E32: np.float32, RHO_S: np.float64}
+           OFFSETS: np.int32, MASK: np.uint8, E32: np.float32, RHO_S: np.float64, PARTNER: np.int32}
 
 
 def build(force=False):
@@ -43,7 +43,8 @@ class Config(C.Structure):
                 ("r_el", C.c_double), ("r_exc", C.c_double), ("r_ion", C.c_double),
                 ("E_exc", C.c_double), ("E_ion", C.c_double),
                 ("gas_vth_ion", C.c_double), ("mass_ratio", C.c_double),
-                ("seed", C.c_uint64), ("flags", C.c_uint32), ("pad_", C.c_uint32)]
+                ("seed", C.c_uint64), ("flags", C.c_uint32), ("pad_", C.c_uint32),
+                ("e_reflect", C.c_double), ("coul_A", C.c_double * 2)]
 
 
 class Moments(C.Structure):
@@ -53,7 +54,8 @@ class Moments(C.Structure):
                 ("absorbed_left", C.c_int64), ("absorbed_right", C.c_int64),
                 ("injected", C.c_int64), ("n_candidates", C.c_int64),
                 ("n_events", C.c_int64 * 4), ("births", C.c_int64),
-                ("dropped", C.c_int64), ("over_cap", C.c_int64)]
+                ("dropped", C.c_int64), ("over_cap", C.c_int64),
+                ("reflected", C.c_int64), ("n_pairs", C.c_int64)]
 
 
 _lib = None
@@ -76,6 +78,9 @@ def make_config(params):
               "omega_dt", "see_gamma", "see_vth", "r_el", "r_exc", "r_ion", "E_exc", "E_ion",
               "gas_vth_ion", "mass_ratio", "seed", "flags"):
         setattr(c, k, params[k])
+    c.e_reflect = params.get("e_reflect", 0.0)
+    for s, a in enumerate(params.get("coul_A", [])):
+        c.coul_A[s] = a
     for s, sp in enumerate(params["species"]):
         for k in ("kappa", "c_eV", "P0", "inv_g_cap", "capacity", "charge_sign", "mcc_kind"):
             setattr(c.sp[s], k, sp[k])

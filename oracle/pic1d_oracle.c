@@ -54,6 +54,8 @@
 #define STREAM_NULL 0u /* + species index */
 #define STREAM_COLL 2u /* + species index */
 #define STREAM_SEE 4u
+#define STREAM_REFL 5u /* electron reflection at the walls (f4) */
+#define STREAM_COUL 6u /* + species index: binary Coulomb collisions inside sort cells (f3) */
 
 typedef struct {
     double kappa;     /* signed push constant kappa_s, Eq. 3 (L119) */
@@ -82,6 +84,9 @@ typedef struct {
     uint64_t seed;
     uint32_t flags;
     uint32_t pad_;
+    double e_reflect; /* probability that an electron reaching a wall is reflected (L41; R22) */
+    double coul_A[ORC_MAX_SPECIES]; /* binary collisions in sort cells (L69): <tan^2(theta/2)> =
+                                       coul_A n_cell / u^3, u in cells/step; 0 = off (R23) */
 } orc_config;
 
 typedef struct {
@@ -94,6 +99,8 @@ typedef struct {
     int64_t births;       /* ionisation births appended to this species */
     int64_t dropped;      /* births / injections dropped for lack of capacity */
     int64_t over_cap;     /* candidates with g > g_cap */
+    int64_t reflected;    /* electrons reflected at a wall (f4) */
+    int64_t n_pairs;      /* binary collisions performed (f3) */
 } orc_moments;
 
 typedef struct {
@@ -102,6 +109,7 @@ typedef struct {
     int32_t* src_key;            /* key per pre-sort slot, -1 = absorbed (debug) */
     uint8_t* mask;               /* MCC event per sorted slot */
     int32_t* offsets;            /* n_sc + 1 */
+    int32_t* partner;            /* f3: partner slot of each sorted slot in the last step, -1 = unpaired */
     double* rho_s;               /* nodes (+1 scratch for periodic wrap) */
     int64_t n, n_sorted, n_src;
     orc_moments m; /* cumulative counters live here */
@@ -164,7 +172,7 @@ static void philox_u(const orc_t* o, uint32_t c0, uint32_t stream, uint32_t blk,
 static void free_species(orc_species* s) {
     free(s->x); free(s->vx); free(s->vy); free(s->vz);
     free(s->tx); free(s->tvx); free(s->tvy); free(s->tvz);
-    free(s->src_key); free(s->mask); free(s->offsets); free(s->rho_s);
+    free(s->src_key); free(s->mask); free(s->offsets); free(s->rho_s); free(s->partner);
     memset(s, 0, sizeof(*s));
 }
 
@@ -196,6 +204,7 @@ int oracle_create(const orc_config* cfg, orc_t** out) {
         p->mask = calloc(cap, 1);
         p->offsets = calloc((size_t)o->n_sc + 1, 4);
         p->rho_s = calloc((size_t)o->nodes + 1, 8);
+        p->partner = malloc(cap * 4);
     }
     o->rho = calloc((size_t)o->nodes + 1, 8);
     o->phi = calloc((size_t)o->nodes + 1, 8);
@@ -444,6 +453,73 @@ static void mcc(orc_t* o) {
     }
 }
 
+/* ---- step 6b (f3): binary Coulomb collisions inside sort cells (L69, L75, L221, L259: the reason
+ * the paper sorts finely; it does not implement them).  Takizuka & Abe's binary collision model
+ * (J. Comput. Phys. 25 (1977) 205), like particles of one species (equal mass, equal weight):
+ * the n particles of a sort cell are paired; a pair with relative velocity u = v_a - v_b is
+ * scattered by the angle theta, tan(theta/2) = delta ~ N(0, <delta^2>),
+ * <delta^2> = coul_A n / u^3 (coul_A = q^4 w lnLambda dt / (8 pi eps0^2 m_r^2 V_cell), m_r = m/2,
+ * in normalised units, computed by the caller), azimuth phi uniform; u is rotated, each partner takes
+ * half of the change: momentum and energy of the pair are conserved.
+ * Pairing (R23; the paper gives none, Takizuka-Abe pair at random): a random affine
+ * permutation pi(k) = (a k + b) mod n of the cell's sorted slots, a coprime to n, from
+ * philox(cell, step, COUL + s, 0); pairs are (pi(2m), pi(2m+1)); for odd n slot pi(n-1) sits out. */
+static uint32_t gcd_u32(uint32_t a, uint32_t b) {
+    while (b) { uint32_t t = a % b; a = b; b = t; }
+    return a;
+}
+
+static void coulomb(orc_t* o) {
+    const orc_config* c = &o->cfg;
+    for (int s = 0; s < c->n_species; ++s) {
+        orc_species* p = &o->sp[s];
+        float A = (float)c->coul_A[s];
+        for (int64_t i = 0; i < p->n_sorted; ++i) p->partner[i] = -1;
+        if (!(A > 0.0f)) continue;
+        for (int k = 0; k < o->n_sc; ++k) {
+            uint32_t off = (uint32_t)p->offsets[k], n = (uint32_t)(p->offsets[k + 1] - p->offsets[k]);
+            if (n < 2) continue;
+            uint32_t w[4];
+            philox4x32_10((uint32_t)k, o->step, STREAM_COUL + (uint32_t)s, 0u, (uint32_t)c->seed,
+                          (uint32_t)(c->seed >> 32), w);
+            uint32_t a = n > 2 ? 1u + w[0] % (n - 1u) : 1u; /* in [1, n) */
+            while (gcd_u32(a, n) != 1u) a = a + 1u == n ? 1u : a + 1u;
+            uint32_t b = w[1] % n;
+            float fn = (float)n;
+            for (uint32_t m = 0; m + 1 < n; m += 2) {
+                uint32_t ia = off + (uint32_t)(((uint64_t)a * m + b) % n);
+                uint32_t ib = off + (uint32_t)(((uint64_t)a * (m + 1) + b) % n);
+                p->partner[ia] = (int32_t)ib; p->partner[ib] = (int32_t)ia;
+                p->m.n_pairs++;
+                float u4[4];
+                philox_u(o, ia, STREAM_COUL + (uint32_t)s, 1u, u4); /* keyed on the pair's first slot */
+                float ux = p->vx[ia] - p->vx[ib], uy = p->vy[ia] - p->vy[ib], uz = p->vz[ia] - p->vz[ib];
+                float up2 = ux * ux + uy * uy;
+                float u2 = up2 + uz * uz;
+                if (!(u2 > 0.0f)) continue;
+                float uu = sqrtf(u2), up = sqrtf(up2);
+                float var = (A * fn) / (u2 * uu);
+                float delta = sqrtf(var) * (bm_r(u4[0]) * cosf(6.2831855f * u4[1]));
+                float d2 = delta * delta;
+                float sint = (2.0f * delta) / (1.0f + d2);
+                float omc = (2.0f * d2) / (1.0f + d2); /* 1 - cos(theta) */
+                float ph = 6.2831855f * u4[2];
+                float cp = cosf(ph), sp_ = sinf(ph);
+                float dux, duy, duz;
+                if (up > 0.0f) {
+                    dux = ((ux / up) * uz) * (sint * cp) - ((uy / up) * uu) * (sint * sp_) - ux * omc;
+                    duy = ((uy / up) * uz) * (sint * cp) + ((ux / up) * uu) * (sint * sp_) - uy * omc;
+                    duz = -(up * (sint * cp)) - uz * omc;
+                } else {
+                    dux = uu * (sint * cp); duy = uu * (sint * sp_); duz = -(uz * omc);
+                }
+                p->vx[ia] += 0.5f * dux; p->vy[ia] += 0.5f * duy; p->vz[ia] += 0.5f * duz;
+                p->vx[ib] -= 0.5f * dux; p->vy[ib] -= 0.5f * duy; p->vz[ib] -= 0.5f * duz;
+            }
+        }
+    }
+}
+
 /* ---- one full step n -> n+1 ------------------------------------------------------ */
 static void step_once(orc_t* o) {
     const orc_config* c = &o->cfg;
@@ -481,6 +557,24 @@ static void step_once(orc_t* o) {
                 /* rounding of -tiny + N_c, |v| > N_c, or non-finite: back to x = 0 */
                 if (!(x >= 0.0f && x < fNc)) x = 0.0f;
             } else if (!(x >= 0.0f && x < fNc)) {
+                /* f4, electron reflection (L41: "If ... electron reflection are featured, electrons are
+                 * inserted at the boundaries"; R22): with probability e_reflect the electron is
+                 * put back at the mirror position with vx reversed, and stays where it was in the order */
+                if (s == 0 && c->e_reflect > 0.0 && x == x) {
+                    float u[4];
+                    philox_u(o, (uint32_t)i, STREAM_REFL, 0u, u);
+                    if (u[0] < (float)c->e_reflect) {
+                        float xr = x < 0.0f ? -x : (2.0f * fNc) - x;
+                        if (xr >= 0.0f && xr < fNc) {
+                            p->m.reflected++;
+                            p->vx[i] = -p->vx[i];
+                            p->src_key[i] = (int)(xr * o->inv_r);
+                            p->x[w] = xr; p->vx[w] = p->vx[i]; p->vy[w] = p->vy[i]; p->vz[w] = p->vz[i];
+                            ++w;
+                            continue;
+                        }
+                    }
+                }
                 if (x != x) o->error = -4;
                 if (x < 0.0f) p->m.absorbed_left++; else p->m.absorbed_right++;
                 p->src_key[i] = -1;
@@ -545,6 +639,7 @@ static void step_once(orc_t* o) {
     deposit(o);
     field_solve_at(o, o->step + 1u);
     mcc(o);
+    coulomb(o);
     o->step += 1u;
 }
 
@@ -625,7 +720,7 @@ int oracle_moments(orc_t* o, int s, orc_moments* out, double* density, int n_den
 }
 
 /* ---- debug access for the parity harness ------------------------------------------ */
-enum { ORC_X = 0, ORC_VX, ORC_VY, ORC_VZ, ORC_KEYS, ORC_OFFSETS, ORC_MASK, ORC_E32, ORC_RHO_S };
+enum { ORC_X = 0, ORC_VX, ORC_VY, ORC_VZ, ORC_KEYS, ORC_OFFSETS, ORC_MASK, ORC_E32, ORC_RHO_S, ORC_PARTNER };
 
 int64_t oracle_debug_count(orc_t* o, int what, int s) {
     if (!o) return -1;
@@ -633,7 +728,7 @@ int64_t oracle_debug_count(orc_t* o, int what, int s) {
         case ORC_X: case ORC_VX: case ORC_VY: case ORC_VZ: return o->sp[s].n;
         case ORC_KEYS: return o->sp[s].n_src;
         case ORC_OFFSETS: return o->n_sc + 1;
-        case ORC_MASK: return o->sp[s].n_sorted;
+        case ORC_MASK: case ORC_PARTNER: return o->sp[s].n_sorted;
         case ORC_E32: return o->nodes;
         case ORC_RHO_S: return o->nodes;
     }
@@ -655,6 +750,7 @@ int oracle_debug_get(orc_t* o, int what, int s, void* dst, size_t bytes) {
         case ORC_KEYS: src = p->src_key; break;
         case ORC_OFFSETS: src = p->offsets; break;
         case ORC_MASK: src = p->mask; el = 1; break;
+        case ORC_PARTNER: src = p->partner; break;
         case ORC_E32: src = o->E32; break;
         case ORC_RHO_S: src = p->rho_s; el = 8; break;
     }

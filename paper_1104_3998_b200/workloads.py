@@ -43,8 +43,11 @@ def _round_up(n, m):
     return (n + m - 1) // m * m
 
 
+LN_LAMBDA = 10.0           # Coulomb logarithm of the binary collisions (f3)
+
+
 def make_params(cfg_id, n_cells=None, ppc=None, sort_ratio=1.0, courant=False, seed=None,
-                capacity_factor=1.25, flags=0, mcc=None, gamma=None):
+                capacity_factor=1.25, flags=0, mcc=None, gamma=None, coulomb=False, e_reflect=0.0):
     """Normalised parameter dict for config `cfg_id` (optionally scaled by n_cells / ppc).
 
     courant=True gives the Courant-respecting twin (same N_c, ppc, dt; dx = config 0's), see
@@ -67,7 +70,7 @@ def make_params(cfg_id, n_cells=None, ppc=None, sort_ratio=1.0, courant=False, s
     p = dict(cfg_id=cfg_id, name=c["name"], n_cells=Nc, ppc=ppc_, bc=c["bc"], steps=c["steps"],
              n_per_species=n_per_species, sort_ratio=float(sort_ratio),
              sort_inv_ratio=1.0 / float(sort_ratio), seed=int(c["seed"]), flags=int(flags),
-             courant=bool(courant))
+             courant=bool(courant), e_reflect=float(e_reflect), coul_A=[0.0, 0.0])
     # performance hint for the library (PIC1D_FLAG_EQ5_ELECTRONS = 4): electron thermal displacement below
     # one cell per step -- configs 0, 1 and the Courant-respecting twins
     if cfg_id in (0, 1) or courant:
@@ -101,6 +104,12 @@ def make_params(cfg_id, n_cells=None, ppc=None, sort_ratio=1.0, courant=False, s
                             inv_g_cap=1.0 / g_cap, capacity=cap, charge_sign=sign,
                             mcc_kind=kind if c["mcc"] else 0, g_cap=g_cap, nu_max=nu_max))
         vth.append(math.sqrt(QE * T / m) * dt / dx)
+        if coulomb:
+            # Takizuka-Abe: <tan^2(theta/2)> = q^4 n_L lnL dt / (8 pi eps0^2 m_r^2 u^3), m_r = m / 2, with
+            # n_L = n_cell w / (A_e r dx) and u in cells/step: coul_A multiplies n_cell / u^3
+            m_r = 0.5 * m
+            p["coul_A"][len(vth) - 1] = (QE ** 4 * LN_LAMBDA * dt * w / (8.0 * math.pi * EPS0 ** 2 * m_r ** 2 * A_E * sort_ratio * dx)
+                                         * (dt / dx) ** 3)
     sig_cap_e = SIG_EL + SIG_EXC0 * (1 - E_EXC / E_CAP) + SIG_ION0 * (1 - E_ION / E_CAP)
     p.update(n_species=2, background_rho=0.0,
              V0_norm=c["V0"] * EPS0 * A_E / (QE * w * dx),

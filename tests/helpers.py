@@ -9,7 +9,7 @@ from paper_1104_3998_b200 import workloads as W
 def params(cfg_id=0, **kw):
     over = {k: kw.pop(k) for k in list(kw) if k in (
         "bc", "background_rho", "V0_norm", "omega_dt", "see_gamma", "see_vth", "r_el", "r_exc",
-        "r_ion", "E_exc", "E_ion", "gas_vth_ion", "mass_ratio", "n_species")}
+        "r_ion", "E_exc", "E_ion", "gas_vth_ion", "mass_ratio", "n_species", "coul_A")}
     sp_over = kw.pop("species_over", None)
     p = copy.deepcopy(W.make_params(cfg_id, **kw))
     p.update(over)

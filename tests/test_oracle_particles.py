@@ -204,6 +204,62 @@ def test_periodic_clamp_faster_than_a_box_length_and_nan():
     assert o.debug_get(O.X).tolist() == [0.0] and o.moments(0)["count"] == 1
 
 
+# ---- f4: electron reflection at the walls (L41; R22) ---------------------------------------
+def test_electron_reflection_mirror_positions_order_and_binomial():
+    Nc, n = 32, 30000
+    rng = np.random.default_rng(4)
+    xe = np.where(np.arange(n) % 2 == 0, 0.25, Nc - 0.5).astype(np.float32)
+    ve = np.where(np.arange(n) % 2 == 0, -1.0, 2.0).astype(np.float32)      # x' = -0.75 / N_c + 1.5: all cross a wall
+    tag = np.arange(n, dtype=np.float32)
+    xi = np.full(100, 0.25, np.float32)
+    vi = np.full(100, -1.0, np.float32)                                        # ions cross too: never reflected
+    for R in (1.0, 0.3, 0.0):
+        p = params(2, n_cells=Nc, ppc=1, mcc=False, gamma=0.0, capacity_factor=1200, e_reflect=R)
+        for s in range(2):
+            p["species"][s]["kappa"] = 0.0
+        o = O.Oracle(p)
+        load(o, [(xe, ve, tag, tag), (xi, vi, 0 * xi, 0 * xi)])
+        o.step(1)
+        me, mi = o.moments(0), o.moments(1)
+        assert mi["count"] == 0 and mi["reflected"] == 0 and mi["absorbed_left"] == 100
+        assert me["reflected"] + me["absorbed_left"] + me["absorbed_right"] == n and me["count"] == me["reflected"]
+        if R == 1.0:
+            assert me["reflected"] == n
+        elif R == 0.0:
+            assert me["reflected"] == 0
+        else:
+            assert abs(me["reflected"] - R * n) < 4 * np.sqrt(n * R * (1 - R))
+            assert abs(me["absorbed_left"] - (1 - R) * n / 2) < 4 * np.sqrt(n / 2 * R * (1 - R))
+        x, vx, tg = o.debug_get(O.X), o.debug_get(O.VX), o.debug_get(O.VY)
+        left = tg % 2 == 0
+        assert np.all(x[left] == 0.75) and np.all(vx[left] == 1.0)             # mirror of -0.75, vx reversed
+        assert np.all(x[~left] == Nc - 1.5) and np.all(vx[~left] == -2.0)      # mirror of N_c + 1.5 at the wall N_c
+        assert np.all(np.diff(tg[left]) > 0) and np.all(np.diff(tg[~left]) > 0)  # survivors keep their order
+    # a particle flung further than a box length beyond the wall is absorbed even with R = 1
+    p = params(2, n_cells=Nc, ppc=1, mcc=False, gamma=0.0, e_reflect=1.0)
+    p["species"][0]["kappa"] = 0.0
+    o = O.Oracle(p)
+    z = np.zeros(0, np.float32)
+    load(o, [(np.array([1.0, 1.0], np.float32), np.array([-40.0, -3.0], np.float32), np.zeros(2, np.float32),
+              np.zeros(2, np.float32)), (z, z, z, z)])
+    o.step(1)
+    assert o.moments(0)["count"] == 1 and o.debug_get(O.X).tolist() == [2.0] and o.moments(0)["absorbed_left"] == 1
+
+
+def test_reflecting_walls_conserve_electrons_and_their_energy():
+    p = params(2, n_cells=64, ppc=50, mcc=False, gamma=0.0, e_reflect=1.0)
+    from paper_1104_3998_b200 import workloads as W
+    parts = W.make_particles(p)
+    for s in range(2):
+        p["species"][s]["kappa"] = 0.0          # free streaming between two mirrors
+    o = O.Oracle(p)
+    load(o, parts)
+    e0 = o.moments(0)["sum_v2"]
+    o.step(30)
+    m = o.moments(0)
+    assert m["count"] == 64 * 50 and m["reflected"] > 200 and abs(m["sum_v2"] / e0 - 1) < 1e-12
+
+
 # ---- moments / EEDF (diagnostics of pic1d_moments) ---------------------------------------------
 def test_moments_and_eedf_against_numpy():
     """oracle_moments() against numpy on the arrays debug_get returns: sums of v, |v|^2, |v|^4 over ALL
