@@ -100,6 +100,12 @@ typedef struct pic1d_config {
     uint64_t seed;         /* Philox key */
     uint32_t flags;        /* PIC1D_FLAG_* */
     uint32_t pad_;
+    double e_reflect;      /* probability that an electron reaching a wall is reflected instead of absorbed: mirror
+                              position, vx reversed, place in the order kept (L41: "If ... electron reflection are
+                              featured, electrons are inserted at the boundaries"); 0 = off */
+    double coul_A[PIC1D_MAX_SPECIES]; /* binary Coulomb collisions between the like particles of a sort cell (L69, L75,
+                              L221, L259; Takizuka-Abe): <tan^2(theta/2)> = coul_A n_cell / u^3 with u in cells/step,
+                              coul_A = q^4 w lnLambda dt / (8 pi eps0^2 m_r^2 A_e r dx) (dt/dx)^3, m_r = m/2; 0 = off */
 } pic1d_config_t;
 
 typedef struct pic1d_moments {
@@ -113,6 +119,8 @@ typedef struct pic1d_moments {
     int64_t births;       /* cumulative ionisation births appended to this species */
     int64_t dropped;      /* cumulative births / injections dropped for lack of capacity */
     int64_t over_cap;     /* cumulative candidates with g > g_cap */
+    int64_t reflected;    /* cumulative electrons reflected at a wall */
+    int64_t n_pairs;      /* cumulative binary Coulomb collisions */
 } pic1d_moments_t;
 
 /*
@@ -194,7 +202,8 @@ enum pic1d_debug_what {
     PIC1D_DBG_MASK = 6,    /* uint8 per sorted slot: MCC event of the last step (needs CAPTURE) */
     PIC1D_DBG_E32 = 7,     /* float[n_nodes]: the field the next push will gather */
     PIC1D_DBG_RHO_S = 8,   /* double[n_nodes]: rho_s of the last deposit */
-    PIC1D_DBG_TILE_W = 9   /* int32 per tile of the last sort: width (sort cells) of the tile's key window */
+    PIC1D_DBG_TILE_W = 9,  /* int32 per tile of the last sort: width (sort cells) of the tile's key window */
+    PIC1D_DBG_PARTNER = 10 /* int32 per sorted slot: partner of the last step's binary collisions, -1 = none (needs CAPTURE) */
 };
 int pic1d_debug_count(pic1d_t* h, int what, int species, int64_t* count_out);
 int pic1d_debug_get(pic1d_t* h, int what, int species, void* dst, size_t bytes);

@@ -19,6 +19,7 @@
 #include "pic1d_sort.cuh"
 #include "pic1d_sort_warp.cuh"
 #include "pic1d_grid.cuh"
+#include "pic1d_coulomb.cuh"
 
 namespace {
 
@@ -30,7 +31,7 @@ struct SpeciesHost {
     bool warp_tiles;  // the species obeys Eq. 5: barrier-free warp-tile kernels (pic1d_sort_warp.cuh)
     int *tile_lo, *tile_w, *tile_off, *tile_dead, *grp_lo, *grp_hi, *pool;
     int pool_size, pool_stride, pool_fixed;
-    int *hist, *offsets, *keys_dbg;
+    int *hist, *offsets, *keys_dbg, *partner;
     uint8_t* mask;
     double *part, *side, *rho_s;
     int n_mcc_tiles;
@@ -183,9 +184,11 @@ size_t layout(pic1d* h, char* base) {
         p.offsets = carve<int>(base, off, h->n_sc + 1);
         p.keys_dbg = nullptr;
         p.mask = nullptr;
+        p.partner = nullptr;
         if (c.flags & PIC1D_FLAG_CAPTURE) {
             p.keys_dbg = carve<int>(base, off, p.capacity);
             p.mask = carve<uint8_t>(base, off, p.capacity);
+            if (c.coul_A[s] > 0.0) p.partner = carve<int>(base, off, p.capacity);
         }
         p.part = carve<double>(base, off, (size_t)h->n_dep_blocks * h->G);
         p.side = carve<double>(base, off, h->n_dep_blocks);
@@ -261,6 +264,8 @@ SortArgs sort_args(pic1d* h, int s) {
     a.fNc = (float)h->cfg.n_cells; a.inv_r = h->inv_r; a.Nc = h->cfg.n_cells; a.n_sc = h->n_sc;
     a.shift = 0; a.WA = h->WA;
     a.m = mcc_params(h, s);
+    a.rp.prob = (s == 0 && h->cfg.bc == 0) ? (float)h->cfg.e_reflect : 0.0f;
+    a.rp.k0 = (uint32_t)h->cfg.seed; a.rp.k1 = (uint32_t)(h->cfg.seed >> 32);
     return a;
 }
 
@@ -442,6 +447,16 @@ void enqueue_mcc(pic1d* h, cudaStream_t st) {
             k_mcc_births<<<h->num_sms * 4, PIC1D_NT, 0, st>>>(m);
             mark(h, "mcc_births", s);
         }
+    }
+    for (int s = 0; s < c.n_species; ++s) {  // binary collisions inside the sort cells (after the MCC, like the oracle)
+        if (!(c.coul_A[s] > 0.0)) continue;
+        SpeciesHost& p = h->sp[s];
+        CoulombArgs ca;
+        ca.vx = p.buf[p.cur][1]; ca.vy = p.buf[p.cur][2]; ca.vz = p.buf[p.cur][3];
+        ca.offsets = p.offsets; ca.partner = p.partner; ca.st = h->st; ca.s = s; ca.n_sc = h->n_sc;
+        ca.A = (float)c.coul_A[s]; ca.k0 = (uint32_t)c.seed; ca.k1 = (uint32_t)(c.seed >> 32);
+        k_coulomb<<<std::min(h->n_sc, h->num_sms * 8), PIC1D_NT, 0, st>>>(ca);
+        mark(h, "coulomb", s);
     }
 }
 
@@ -732,6 +747,7 @@ int pic1d_moments(pic1d_t* h, int s, pic1d_moments_t* out, double* density, int 
     out->injected = (int64_t)d.injected; out->n_candidates = (int64_t)d.n_candidates;
     for (int k = 0; k < 4; ++k) out->n_events[k] = (int64_t)d.n_events[k];
     out->births = (int64_t)d.births; out->dropped = (int64_t)d.dropped; out->over_cap = (int64_t)d.over_cap;
+    out->reflected = (int64_t)d.reflected; out->n_pairs = (int64_t)d.n_pairs;
     return sticky_code(st.err);
 }
 
@@ -750,7 +766,7 @@ int pic1d_debug_count(pic1d_t* h, int what, int s, int64_t* count_out) {
         case PIC1D_DBG_X: case PIC1D_DBG_VX: case PIC1D_DBG_VY: case PIC1D_DBG_VZ: *count_out = st.sp[s].n_live; break;
         case PIC1D_DBG_KEYS: *count_out = st.sp[s].n_src; break;
         case PIC1D_DBG_OFFSETS: *count_out = h->n_sc + 1; break;
-        case PIC1D_DBG_MASK: *count_out = st.sp[s].n_sorted; break;
+        case PIC1D_DBG_MASK: case PIC1D_DBG_PARTNER: *count_out = st.sp[s].n_sorted; break;
         case PIC1D_DBG_E32: case PIC1D_DBG_RHO_S: *count_out = h->nodes; break;
         case PIC1D_DBG_TILE_W: *count_out = st.sp[s].n_tiles; break;
         default: return PIC1D_ERR_ARG;
@@ -774,6 +790,7 @@ int pic1d_debug_get(pic1d_t* h, int what, int s, void* dst, size_t bytes) {
         case PIC1D_DBG_E32: src = h->E32; break;
         case PIC1D_DBG_RHO_S: src = p.rho_s; el = 8; break;
         case PIC1D_DBG_TILE_W: src = p.tile_w; break;
+        case PIC1D_DBG_PARTNER: src = p.partner; break;
     }
     if (!src || bytes < (size_t)n * el) return PIC1D_ERR_ARG;
     if (n > 0 && !ck(h, cudaMemcpyAsync(dst, src, (size_t)n * el, cudaMemcpyDeviceToHost, h->stream))) return PIC1D_ERR_CUDA;

@@ -1,0 +1,86 @@
+// pic1d_coulomb.cuh -- binary Coulomb collisions inside sort cells.
+//
+// The paper names them as THE reason for fine sorting ("allows for a straightforward and fast implementation
+// of nonlinear collision processes (i.e. Coulomb collisions) through the binary collisions"; L75,
+// L221, L259) but does not implement them.  The sorted per-cell ranges offsets[k] .. offsets[k+1] built by the
+// fine sort are exactly the data structure the binary-collision model of Takizuka & Abe (J. Comput. Phys. 25
+// (1977) 205) needs: the n particles of a sort cell are paired, a pair with relative velocity u is scattered by
+// theta with tan(theta/2) = delta ~ N(0, coul_A n / u^3) and a uniform azimuth, each partner takes half of the
+// change of u (like particles: equal mass and weight), so momentum and energy of every pair are conserved.
+// Pairing (R23): a random affine permutation pi(m) = (a m + b) mod n of the cell's sorted slots, a
+// coprime to n, from philox(cell, step, COUL + s, 0); pairs (pi(2m), pi(2m+1)); for odd n slot pi(n-1) sits out.
+// One block per sort cell, one thread per pair; the cell's velocities (12 B x n) are gathered through L1.
+// fp32 operations in the order the oracle states them (-fmad=false: nothing is contracted).
+#pragma once
+#include "pic1d_device.cuh"
+#include "pic1d_mcc.cuh"
+
+struct CoulombArgs {
+    float *vx, *vy, *vz;   // the species' sorted buffer
+    const int* offsets;    // [n_sc + 1]
+    int* partner;          // optional (PIC1D_FLAG_CAPTURE): partner slot per sorted slot, -1 = sits out
+    DevState* st;
+    int s, n_sc;
+    float A;               // coul_A
+    uint32_t k0, k1;
+};
+
+__device__ __forceinline__ unsigned gcd_u32(unsigned a, unsigned b) {
+    while (b) { const unsigned t = a % b; a = b; b = t; }
+    return a;
+}
+
+__global__ void __launch_bounds__(PIC1D_NT) k_coulomb(CoulombArgs a) {
+    const int tid = threadIdx.x, lane = tid & 31;
+    const uint32_t step = a.st->step;
+    const uint32_t stream = STREAM_COUL + (uint32_t)a.s;
+    unsigned n_pairs = 0;
+    for (int k = blockIdx.x; k < a.n_sc; k += gridDim.x) {
+        const unsigned off = (unsigned)a.offsets[k], n = (unsigned)(a.offsets[k + 1] - a.offsets[k]);
+        if (n < 2u) {
+            if (a.partner && n == 1u && tid == 0) a.partner[off] = -1;
+            continue;
+        }
+        uint32_t w[4];
+        philox4x32_10((uint32_t)k, step, stream, 0u, a.k0, a.k1, w);  // every thread: the cell's permutation
+        unsigned am = n > 2u ? 1u + w[0] % (n - 1u) : 1u;             // in [1, n)
+        while (gcd_u32(am, n) != 1u) am = am + 1u == n ? 1u : am + 1u;
+        const unsigned bm = w[1] % n;
+        const float fn = (float)n;
+        if (a.partner && (n & 1u) && tid == 0) a.partner[off + (unsigned)(((ull)am * (n - 1u) + bm) % n)] = -1;
+        for (unsigned m = 2u * tid; m + 1u < n; m += 2u * PIC1D_NT) {
+            const unsigned ia = off + (unsigned)(((ull)am * m + bm) % n);
+            const unsigned ib = off + (unsigned)(((ull)am * (m + 1u) + bm) % n);
+            if (a.partner) { a.partner[ia] = (int)ib; a.partner[ib] = (int)ia; }
+            ++n_pairs;
+            const float vxa = a.vx[ia], vya = a.vy[ia], vza = a.vz[ia];
+            const float vxb = a.vx[ib], vyb = a.vy[ib], vzb = a.vz[ib];
+            const float ux = vxa - vxb, uy = vya - vyb, uz = vza - vzb;
+            const float up2 = ux * ux + uy * uy;
+            const float u2 = up2 + uz * uz;
+            if (!(u2 > 0.0f)) continue;
+            uint32_t r[4];
+            philox4x32_10(ia, step, stream, 1u, a.k0, a.k1, r);  // keyed on the pair's first slot
+            const float uu = sqrtf(u2), up = sqrtf(up2);
+            const float var = (a.A * fn) / (u2 * uu);
+            const float delta = sqrtf(var) * (bm_r(u01(r[0])) * cosf(6.2831855f * u01(r[1])));
+            const float d2 = delta * delta;
+            const float sint = (2.0f * delta) / (1.0f + d2);
+            const float omc = (2.0f * d2) / (1.0f + d2);  // 1 - cos(theta)
+            const float ph = 6.2831855f * u01(r[2]);
+            const float cp = cosf(ph), sp = sinf(ph);
+            float dux, duy, duz;
+            if (up > 0.0f) {
+                dux = ((ux / up) * uz) * (sint * cp) - ((uy / up) * uu) * (sint * sp) - ux * omc;
+                duy = ((uy / up) * uz) * (sint * cp) + ((ux / up) * uu) * (sint * sp) - uy * omc;
+                duz = -(up * (sint * cp)) - uz * omc;
+            } else {
+                dux = uu * (sint * cp); duy = uu * (sint * sp); duz = -(uz * omc);
+            }
+            a.vx[ia] = vxa + 0.5f * dux; a.vy[ia] = vya + 0.5f * duy; a.vz[ia] = vza + 0.5f * duz;
+            a.vx[ib] = vxb - 0.5f * dux; a.vy[ib] = vyb - 0.5f * duy; a.vz[ib] = vzb - 0.5f * duz;
+        }
+    }
+    n_pairs = __reduce_add_sync(0xffffffffu, n_pairs);
+    if (lane == 0 && n_pairs) atomicAdd(&a.st->sp[a.s].n_pairs, (ull)n_pairs);
+}

@@ -15,6 +15,8 @@
 #define STREAM_NULL 0u
 #define STREAM_COLL 2u
 #define STREAM_SEE 4u
+#define STREAM_REFL 5u  // electron reflection at the walls (f4)
+#define STREAM_COUL 6u  // + species: binary Coulomb collisions inside sort cells (f3)
 
 // sticky error bits in DevState::err
 #define ERRBIT_CAPACITY 1u
@@ -38,6 +40,7 @@ struct DevSpecies {
     int ticket2;   // dynamic tile counter of the scatter kernel
     int scan_done; // bin blocks of k_bin_scan that have finished (the last one scans the histogram)
     ull absorbed_left, absorbed_right, injected, n_candidates, n_events[4], births, dropped, over_cap;
+    ull reflected, n_pairs;  // f4: electrons reflected at a wall; f3: binary collisions performed
 };
 
 struct DevState {
@@ -97,14 +100,22 @@ __device__ __forceinline__ int warp_sum(int v) {
     return v;
 }
 
+// f4, electron reflection at the walls (L41; R22): prob = 0 switches it off
+struct ReflP {
+    float prob;
+    uint32_t k0, k1;
+};
+
 // Gather + leapfrog push + boundary + sort key for ONE particle (PAPER.md L35, L87, L150-156,
 // Eq. 3-4; boundary L41; key L63-67).  Used verbatim by the counting pass and by the scatter pass,
-// so both see bit-identical x, vx and key.
+// so both see bit-identical x, vx and key.  slot = the particle's source slot (keys the reflection draw);
+// n_refl counts the reflections.
 //   key >= 0 : sort cell;  -1 : absorbed at the left wall;  -2 : absorbed at the right wall / NaN
 template <int BC>
 __device__ __forceinline__ int push_particle(float& x, float& vx, bool do_push,
                                              const float* __restrict__ E32, float kappa, int Nc,
-                                             float fNc, float inv_r, int shift) {
+                                             float fNc, float inv_r, int shift,
+                                             const ReflP& rp, uint32_t step, unsigned slot, int& n_refl) {
     if (do_push) {
         int j = (int)x;  // "single type casting operation", L87
         float f = __fsub_rn(x, (float)j);
@@ -120,7 +131,16 @@ __device__ __forceinline__ int push_particle(float& x, float& vx, bool do_push,
         if (x >= fNc) x = __fsub_rn(x, fNc);
         if (!(x >= 0.0f && x < fNc)) x = 0.0f;  // rounding of -tiny + N_c, |v| > N_c, non-finite
     } else if (!(x >= 0.0f && x < fNc)) {
-        return x < 0.0f ? -1 : -2;
+        bool back = false;
+        if (rp.prob > 0.0f && do_push && x == x) {  // with probability prob: mirror position, vx reversed
+            uint32_t w[4];
+            philox4x32_10(slot, step, STREAM_REFL, 0u, rp.k0, rp.k1, w);
+            if (u01(w[0]) < rp.prob) {
+                const float xr = x < 0.0f ? -x : __fsub_rn(__fmul_rn(2.0f, fNc), x);
+                if (xr >= 0.0f && xr < fNc) { x = xr; vx = -vx; back = true; ++n_refl; }
+            }
+        }
+        if (!back) return x < 0.0f ? -1 : -2;
     }
     return ((int)__fmul_rn(x, inv_r)) >> shift;  // shift > 0 only in the coarse pass of a load
 }

@@ -44,6 +44,7 @@ struct SortArgs {
     int shift;  // key = sort cell >> shift (0 except in the coarse pass of an unsorted load)
     int WA;     // sub-window (bins) the scatter kernel ranks at a time in shared memory (a multiple of 8)
     MccP m;     // collision model of the species, for the scatter kernels that fold the MCC in
+    ReflP rp;        // electron reflection at the walls (prob = 0: off)
     int null_first;  // k_bin_scan: blocks from (bin blocks + null_first) on compute the null-test bit mask
 };
 
@@ -64,6 +65,8 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
     const int WA = a.WA;
     DevSpecies& sp = a.st->sp[a.s];
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
+    const uint32_t step = a.st->step;
+    int n_refl = 0;
     for (int i = tid; i < WA; i += PIC1D_NT) s_hist[i] = 0;
     if (tid < 2) { s_lohi[tid][0] = 0x7fffffff; s_lohi[tid][1] = -1; s_dead[tid][0] = 0; s_dead[tid][1] = 0; }
     __syncthreads();
@@ -88,7 +91,7 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
                 float xs[4] = {X[v].x, X[v].y, X[v].z, X[v].w}, vs[4] = {VX[v].x, VX[v].y, VX[v].z, VX[v].w};
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    const int key = push_particle<BC>(xs[c], vs[c], true, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                    const int key = push_particle<BC>(xs[c], vs[c], true, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift, a.rp, step, (unsigned)(base + (v * PIC1D_NT + tid) * 4 + c), n_refl);
                     ulo = min(ulo, (unsigned)key); hi = max(hi, key); smin = min(smin, key);
                     if (key == -2) nonfinite |= (xs[c] != xs[c]);
                     keys[v * 4 + c] = key;
@@ -110,7 +113,7 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
                     int key = -3;  // no particle
                     smin = min(smin, i < n_src ? 0 : -3);
                     if (i < n_src) {
-                        key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                        key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift, a.rp, step, (unsigned)i, n_refl);
                         ulo = min(ulo, (unsigned)key); hi = max(hi, key); smin = min(smin, key);
                         if (key == -2) nonfinite |= (xs[c] != xs[c]);
                         if (a.keys_dbg) a.keys_dbg[i] = key >= 0 ? key : -1;
@@ -163,6 +166,7 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
             }
             a.tile_lo[tile] = lo; a.tile_w[tile] = off >= 0 ? w : 0; a.tile_off[tile] = off;
             a.tile_dead[tile] = dl + dr;
+            if (off < 0) atomicAdd(&sp.dropped, (ull)(min(T, n_src - base) - dl - dr));  // the tile is lost (sticky error)
             if (dl) atomicAdd(&sp.absorbed_left, (ull)dl);
             if (dr) atomicAdd(&sp.absorbed_right, (ull)dr);
             // reset the OTHER buffer for the next tile (nobody touches it before the next barrier)
@@ -185,6 +189,10 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
             __syncthreads();
         }
         if (w == 0) __syncthreads();  // keep the double buffer two barriers apart
+    }
+    if (a.rp.prob > 0.0f) {  // reflections are counted here only (the scatter repeats the same decisions)
+        n_refl = __reduce_add_sync(0xffffffffu, n_refl);
+        if (lane == 0 && n_refl) atomicAdd(&sp.reflected, (ull)n_refl);
     }
 }
 
@@ -483,6 +491,7 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
     DevSpecies& sp = a.st->sp[a.s];
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
     const uint32_t step = a.st->step;
+    int n_refl = 0;  // (counted by the counting pass)
     MccCount mc = {0u, 0u, 0u};
     for (int i = tid; i < cnt_words; i += PIC1D_NT) reinterpret_cast<unsigned*>(s_cnt)[i] = 0u;  // counters are zero between tiles
     if (tid == 0) s_tile = atomicAdd(&sp.ticket2, 1);
@@ -510,20 +519,14 @@ __global__ void __launch_bounds__(PIC1D_NT, (STAGE ? 3 : (ROWS <= 4 ? 6 : 4))) k
         // absolute base of the tile per bin of the first sub-window: in flight together with the particles
         for (int i = tid; i < min(WA, wtot); i += PIC1D_NT)
             s_base[i] = (unsigned)(a.offsets[lo + i] + __ldcg(a.pool + off + i));
-        int n_lost = 0;
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
             const int i = base + r * 32;
             rel[r] = -1;
             if (full || i < n_src) {
-                const int key = push_particle<BC>(x[r], vx[r], full || i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                const int key = push_particle<BC>(x[r], vx[r], full || i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift, a.rp, step, (unsigned)i, n_refl);
                 rel[r] = key >= 0 ? key - lo : -1;
-                n_lost += (off < 0 && key >= 0) ? 1 : 0;
             }
-        }
-        if (off < 0) {  // block-uniform, after a sticky workspace error only: count what is lost
-            n_lost = __reduce_add_sync(0xffffffffu, n_lost);
-            if (lane == 0 && n_lost) atomicAdd(&sp.dropped, (ull)n_lost);
         }
         const bool staged = STAGE && wtot <= WA && wtot >= T / 64;  // block-uniform
         for (int sub = 0; sub < wtot; sub += WA) {

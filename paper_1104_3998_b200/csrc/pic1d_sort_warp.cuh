@@ -28,6 +28,8 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count_w(SortArgs a) {
     DevSpecies& sp = a.st->sp[a.s];
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
     const int n_warps = gridDim.x * PIC1D_NWARP;
+    const uint32_t step = a.st->step;
+    int n_refl = 0;
     for (int tile = blockIdx.x * PIC1D_NWARP + wp; tile < n_tiles; tile += n_warps) {
         const int base = tile * PIC1D_TW;
         int keys[8];
@@ -48,7 +50,7 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count_w(SortArgs a) {
                 float xs[4] = {X[v].x, X[v].y, X[v].z, X[v].w}, vs[4] = {VX[v].x, VX[v].y, VX[v].z, VX[v].w};
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    const int key = push_particle<BC>(xs[c], vs[c], true, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                    const int key = push_particle<BC>(xs[c], vs[c], true, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift, a.rp, step, (unsigned)(base + v * 128 + lane * 4 + c), n_refl);
                     ulo = min(ulo, (unsigned)key); hi = max(hi, key); smin = min(smin, key);
                     if (key == -2) nonfinite |= (xs[c] != xs[c]);
                     keys[v * 4 + c] = key;
@@ -70,7 +72,7 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count_w(SortArgs a) {
                     int key = -3;  // no particle
                     smin = min(smin, i < n_src ? 0 : -3);
                     if (i < n_src) {
-                        key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                        key = push_particle<BC>(xs[c], vs[c], i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift, a.rp, step, (unsigned)i, n_refl);
                         ulo = min(ulo, (unsigned)key); hi = max(hi, key); smin = min(smin, key);
                         if (key == -2) nonfinite |= (xs[c] != xs[c]);
                         if (a.keys_dbg) a.keys_dbg[i] = key >= 0 ? key : -1;
@@ -111,6 +113,7 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count_w(SortArgs a) {
             }
             a.tile_lo[tile] = lo; a.tile_w[tile] = off >= 0 ? w : 0; a.tile_off[tile] = off;
             a.tile_dead[tile] = dl + dr;
+            if (off < 0) atomicAdd(&sp.dropped, (ull)(min(PIC1D_TW, n_src - base) - dl - dr));  // the tile is lost (sticky error)
             if (dl) atomicAdd(&sp.absorbed_left, (ull)dl);
             if (dr) atomicAdd(&sp.absorbed_right, (ull)dr);
         }
@@ -136,6 +139,10 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count_w(SortArgs a) {
                 if (keys[q] >= 0) atomicAdd(&a.pool[off + keys[q] - lo], 1);
         }
     }
+    if (a.rp.prob > 0.0f) {  // reflections are counted here only (the scatter repeats the same decisions)
+        n_refl = __reduce_add_sync(0xffffffffu, n_refl);
+        if (lane == 0 && n_refl) atomicAdd(&sp.reflected, (ull)n_refl);
+    }
 }
 
 // MCCK != 0: the species' null-collision MCC is folded in (mcc_lane: the destination slot is the particle id)
@@ -149,13 +156,11 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_push_scatter_w(SortArgs a) {
     const int n_warps = gridDim.x * PIC1D_NWARP;
     unsigned* cur = s_cur[wp];
     const uint32_t step = a.st->step;
+    int n_refl = 0;  // (counted by the counting pass)
     MccCount mc = {0u, 0u, 0u};
     for (int tile = blockIdx.x * PIC1D_NWARP + wp; tile < n_tiles; tile += n_warps) {
         const int lo = a.tile_lo[tile], w = a.tile_w[tile], off = a.tile_off[tile];
-        if (off < 0) {  // count pool exhausted (sticky error): the tile is lost, and counted as dropped
-            if (lane == 0) atomicAdd(&sp.dropped, (ull)min(PIC1D_TW, n_src - tile * PIC1D_TW));
-            continue;
-        }
+        if (off < 0) continue;  // count pool exhausted (sticky error): the tile is lost (counted by the counting pass)
         const int base = tile * PIC1D_TW + lane;
         const bool full = tile * PIC1D_TW + PIC1D_TW <= n_push;  // warp-uniform
         const bool narrow = w <= PIC1D_PSW;
@@ -183,7 +188,7 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_push_scatter_w(SortArgs a) {
             const int i = base + r * 32;
             k[r] = -1;
             if (full || i < n_src) {
-                const int key = push_particle<BC>(x[r], vx[r], full || i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift);
+                const int key = push_particle<BC>(x[r], vx[r], full || i < n_push, a.E32, a.kappa, a.Nc, a.fNc, a.inv_r, a.shift, a.rp, step, (unsigned)i, n_refl);
                 k[r] = key >= 0 ? key - lo : (ABS ? w : -1);
                 if (ABS && key == -2) wall |= 1u << r;
             }

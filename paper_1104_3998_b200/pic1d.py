@@ -21,10 +21,10 @@ FLAG_FOLD_ALL = 16
 FLAG_MCC_GATHER = 32
 FLAG_NO_OVERLAP = 64
 FLAG_NO_GRAPH = 128
-DBG_X, DBG_VX, DBG_VY, DBG_VZ, DBG_KEYS, DBG_OFFSETS, DBG_MASK, DBG_E32, DBG_RHO_S, DBG_TILE_W = range(10)
+DBG_X, DBG_VX, DBG_VY, DBG_VZ, DBG_KEYS, DBG_OFFSETS, DBG_MASK, DBG_E32, DBG_RHO_S, DBG_TILE_W, DBG_PARTNER = range(11)
 _DBG_DTYPE = {DBG_X: np.float32, DBG_VX: np.float32, DBG_VY: np.float32, DBG_VZ: np.float32,
               DBG_KEYS: np.int32, DBG_OFFSETS: np.int32, DBG_MASK: np.uint8, DBG_E32: np.float32,
-              DBG_RHO_S: np.float64, DBG_TILE_W: np.int32}
+              DBG_RHO_S: np.float64, DBG_TILE_W: np.int32, DBG_PARTNER: np.int32}
 
 EXPORTS = ["pic1d_workspace_bytes", "pic1d_create", "pic1d_load_particles", "pic1d_step",
            "pic1d_get_rho_phi_E", "pic1d_moments", "pic1d_destroy", "pic1d_n_nodes",
@@ -48,7 +48,8 @@ class Config(C.Structure):
                 ("r_el", C.c_double), ("r_exc", C.c_double), ("r_ion", C.c_double),
                 ("E_exc", C.c_double), ("E_ion", C.c_double),
                 ("gas_vth_ion", C.c_double), ("mass_ratio", C.c_double),
-                ("seed", C.c_uint64), ("flags", C.c_uint32), ("pad_", C.c_uint32)]
+                ("seed", C.c_uint64), ("flags", C.c_uint32), ("pad_", C.c_uint32),
+                ("e_reflect", C.c_double), ("coul_A", C.c_double * 2)]
 
 
 class Moments(C.Structure):
@@ -58,7 +59,8 @@ class Moments(C.Structure):
                 ("absorbed_left", C.c_int64), ("absorbed_right", C.c_int64),
                 ("injected", C.c_int64), ("n_candidates", C.c_int64),
                 ("n_events", C.c_int64 * 4), ("births", C.c_int64),
-                ("dropped", C.c_int64), ("over_cap", C.c_int64)]
+                ("dropped", C.c_int64), ("over_cap", C.c_int64),
+                ("reflected", C.c_int64), ("n_pairs", C.c_int64)]
 
 
 class KernelTime(C.Structure):
@@ -91,6 +93,9 @@ def make_config(params):
               "omega_dt", "see_gamma", "see_vth", "r_el", "r_exc", "r_ion", "E_exc", "E_ion",
               "gas_vth_ion", "mass_ratio", "seed", "flags"):
         setattr(c, k, params[k])
+    c.e_reflect = params.get("e_reflect", 0.0)
+    for s, a in enumerate(params.get("coul_A", [])):
+        c.coul_A[s] = a
     for s, sp in enumerate(params["species"]):
         for k in ("kappa", "c_eV", "P0", "inv_g_cap", "capacity", "charge_sign", "mcc_kind"):
             setattr(c.sp[s], k, sp[k])

@@ -28,7 +28,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_struct_sizes_and_workspace_query():
     lib = G.load_library()
-    assert C.sizeof(G.Config) == 16 + 2 * 48 + 13 * 8 + 8 + 8
+    assert C.sizeof(G.Config) == 16 + 2 * 48 + 13 * 8 + 8 + 8 + 3 * 8
     for cfg in (0, 1, 2):
         c = G.make_config(W.make_params(cfg))
         n = C.c_size_t()

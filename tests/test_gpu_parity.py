@@ -30,10 +30,15 @@ def _mk(p):
     return o, g, p
 
 
-def _vel_err(gv, ov):
+def _vel_err(gv, ov, partner=None):
+    """max over particles of |dv|_inf / |v|; after a binary collision (f3) the scale is the larger speed of the
+    pair: v' = v +- du / 2, and the rounding of du scales with |u| <= |v_a| + |v_b|, not with the own speed"""
     gv = np.stack(gv, 1).astype(np.float64)
     ov = np.stack(ov, 1).astype(np.float64)
     nrm = np.maximum(np.linalg.norm(ov, axis=1), 1e-30)
+    if partner is not None and partner.size:
+        m = partner >= 0
+        nrm[:partner.shape[0]][m] = np.maximum(nrm[:partner.shape[0]][m], nrm[partner[m]])
     return float(np.max(np.abs(gv - ov).max(1) / nrm)) if gv.size else 0.0
 
 
@@ -44,16 +49,19 @@ def compare_state(o, g, p, check_keys=True):
     for s in range(p["n_species"]):
         mo, mg = o.moments(s), g.moments(s)
         for k in ("count", "n_sorted", "absorbed_left", "absorbed_right", "injected", "n_candidates",
-                  "n_events", "births", "dropped", "over_cap"):
+                  "n_events", "births", "dropped", "over_cap", "reflected", "n_pairs"):
             assert mo[k] == mg[k], (s, k, mo[k], mg[k])
         assert np.array_equal(o.debug_get(O.OFFSETS, s), g.debug_get(G.DBG_OFFSETS, s)), s
+        if check_keys and p.get("coul_A", [0, 0])[s] > 0:      # f3: who collided with whom
+            assert np.array_equal(o.debug_get(O.PARTNER, s), g.debug_get(G.DBG_PARTNER, s)), s
         if check_keys:
             assert np.array_equal(o.debug_get(O.KEYS, s), g.debug_get(G.DBG_KEYS, s)), s
             assert np.array_equal(o.debug_get(O.MASK, s), g.debug_get(G.DBG_MASK, s)), s
         ox, gx = o.debug_get(O.X, s), g.debug_get(G.DBG_X, s)
         assert np.array_equal(ox, gx), (s, np.nonzero(ox != gx)[0][:10])
+        part = o.debug_get(O.PARTNER, s) if check_keys and p.get("coul_A", [0, 0])[s] > 0 else None
         ev = _vel_err([g.debug_get(w, s) for w in (G.DBG_VX, G.DBG_VY, G.DBG_VZ)],
-                      [o.debug_get(w, s) for w in (O.VX, O.VY, O.VZ)])
+                      [o.debug_get(w, s) for w in (O.VX, O.VY, O.VZ)], part)
         assert ev <= TOL_V, (s, ev)
         assert rel_linf(g.debug_get(G.DBG_RHO_S, s), o.debug_get(O.RHO_S, s)) <= TOL_RHO
         for k in ("sum_vx", "sum_vy", "sum_vz", "sum_v2", "sum_v4"):
@@ -508,3 +516,48 @@ def test_moments_and_eedf_bit_for_bit():
                 assert abs(mo[k] / mg[k] - 1) <= 1e-12, k
             assert np.array_equal(mo["density"], mg["density"])
     o.close(); g.close()
+
+
+@pytest.mark.parametrize("kw", [dict(cfg_id=2, n_cells=256, ppc=150), dict(cfg_id=2, n_cells=256, ppc=150, courant=True),
+                                dict(cfg_id=3, n_cells=512, ppc=200, sort_ratio=2.0)])
+def test_f4_electron_reflection_at_the_walls(kw):
+    """L41: electrons that reach a wall are reflected with probability e_reflect (mirror position, vx reversed,
+    place in the order kept) -- both sort families, every output compared"""
+    o, g, p = _mk(W.make_params(e_reflect=0.4, **kw))
+    run_compared_steps(o, g, p, 4)
+    assert g.moments(0)["reflected"] > 20 and g.moments(1)["reflected"] == 0
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("kw", [dict(cfg_id=2, n_cells=256, ppc=150), dict(cfg_id=2, n_cells=128, ppc=301, sort_ratio=2.0),
+                                dict(cfg_id=0), dict(cfg_id=3, n_cells=512, ppc=64, sort_ratio=0.5, courant=True)])
+def test_f3_binary_coulomb_collisions_in_sort_cells(kw):
+    """L69 / L259: like-particle binary collisions inside the sort cells (Takizuka-Abe).  The pairing is integer
+    work and must match bit for bit; the scattered velocities to 1e-6.  coul_A is scaled up so that the
+    collisions change the velocities visibly within a few steps."""
+    p = W.make_params(coulomb=True, **kw)
+    p["coul_A"] = [p["coul_A"][0] * 3e4, p["coul_A"][1] * 1e9]
+    o, g, p = _mk(p)
+    v0 = g.debug_get(1, 0).copy()
+    run_compared_steps(o, g, p, 3)
+    for s in range(2):
+        assert g.moments(s)["n_pairs"] > 0
+    assert g.debug_get(10, 0).min() >= -1
+    o.close(); g.close()
+
+
+def test_exhausted_count_pool_is_flagged_and_counted_not_silent():
+    """hot electrons forced through the warp-tile family (wrong Eq. 5 hint): windows far beyond the 32-bin rows
+    exhaust the overflow region; the lost tiles' particles are counted in `dropped` and the sticky workspace
+    error is raised (include/pic1d.h, "Displacement limits")"""
+    from paper_1104_3998_b200 import pic1d as G
+    p = W.make_params(3, n_cells=4096, ppc=700, mcc=False, gamma=0.0)
+    p["vth"] = [600.0, p["vth"][1]]
+    p["flags"] |= G.FLAG_EQ5_ELECTRONS
+    g = G.Pic1D(p)
+    load(g, W.make_particles(p))
+    g.step(1)
+    m = g.moments(0)
+    assert m["sticky"] == G.ERR_WORKSPACE and m["dropped"] > 0
+    assert m["count"] + m["dropped"] + m["absorbed_left"] + m["absorbed_right"] == p["n_per_species"]
+    g.close()
