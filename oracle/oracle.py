@@ -178,3 +178,50 @@ def solve_field(n_cells, bc, rho, phi0=0.0, phiN=0.0):
     lib().oracle_solve_field(C.c_int(n_cells), C.c_int(bc), _fp(rho), C.c_double(phi0),
                              C.c_double(phiN), _fp(phi), _fp(E))
     return phi[:nodes], E[:nodes]
+
+
+class Gapped:
+    """the paper's gapped in-place fine sort (f2), stated step by step in pic1d_oracle.c"""
+
+    def __init__(self, n_cells, sort_inv_ratio, n_max, kappa):
+        self.h = C.c_void_p()
+        rc = lib().oracle_gapped_create(C.c_int(n_cells), C.c_double(sort_inv_ratio), C.c_int(n_max),
+                                        C.c_double(kappa), C.byref(self.h))
+        if rc:
+            raise ValueError("oracle_gapped_create failed")
+        self.n_cells, self.n_max = n_cells, n_max
+        self.n_sc = lib().oracle_gapped_n_sort_cells(self.h)
+
+    def close(self):
+        if self.h:
+            lib().oracle_gapped_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def load(self, x, vx, vy, vz):
+        a = [np.ascontiguousarray(v, dtype=np.float32) for v in (x, vx, vy, vz)]
+        return lib().oracle_gapped_load(self.h, C.c_int64(a[0].shape[0]), *[_fp(v) for v in a])
+
+    def set_E32(self, e32):
+        a = np.ascontiguousarray(e32, dtype=np.float32)
+        assert lib().oracle_gapped_set_E32(self.h, _fp(a), C.c_int(a.shape[0])) == 0
+
+    def step(self):
+        return lib().oracle_gapped_step(self.h)
+
+    def get(self):
+        """(N_i, [x, vx, vy, vz] as (n_sc, n_max) arrays, stats dict)"""
+        N = np.zeros(self.n_sc, np.int32)
+        arr = [np.zeros((self.n_sc, self.n_max), np.float32) for _ in range(4)]
+        st = np.zeros(4, np.int64)
+        rc = lib().oracle_gapped_get(self.h, _fp(N), *[_fp(a) for a in arr], _fp(st))
+        return N, arr, dict(absorbed_left=int(st[0]), absorbed_right=int(st[1]), moved_near=int(st[2]),
+                            moved_far=int(st[3]), error=rc)
+
+
+def cell_multisets(N, arr):
+    """per sort cell: the valid 4-tuples, sorted lexicographically (the order inside a cell is undefined)"""
+    out = []
+    for k in range(N.shape[0]):
+        t = np.stack([a[k, :N[k]] for a in arr], 1)
+        out.append(t[np.lexsort(t.T[::-1])] if t.shape[0] else t)
+    return out

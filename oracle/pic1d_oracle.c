@@ -520,6 +520,20 @@ static void coulomb(orc_t* o) {
     }
 }
 
+/* ---- step 1 for ONE particle: gather (linear weighting, L35) + leapfrog push (L150-156):
+ *   v(t+1/2) = v(t-1/2) + kappa E(x(t));   x(t+1) = x(t) + v(t+1/2)   (L152-154) */
+static void gather_push(const float* E32, float kappa, int Nc, int bc, float* px, float* pvx) {
+    float x = *px;
+    int j = (int)x; /* "single type casting operation", L87 */
+    float f = x - (float)j;
+    int j1 = j + 1;
+    if (bc == 1 && j1 == Nc) j1 = 0;
+    float Ep = fmaf(f, E32[j1] - E32[j], E32[j]);
+    float v = fmaf(kappa, Ep, *pvx);
+    *pvx = v;
+    *px = x + v;
+}
+
 /* ---- one full step n -> n+1 ------------------------------------------------------ */
 static void step_once(orc_t* o) {
     const orc_config* c = &o->cfg;
@@ -530,17 +544,7 @@ static void step_once(orc_t* o) {
     for (int s = 0; s < c->n_species; ++s) {
         orc_species* p = &o->sp[s];
         float kappa = (float)c->sp[s].kappa;
-        for (int64_t i = 0; i < p->n; ++i) {
-            float x = p->x[i];
-            int j = (int)x; /* "single type casting operation", L87 */
-            float f = x - (float)j;
-            int j1 = j + 1;
-            if (c->bc == 1 && j1 == Nc) j1 = 0;
-            float Ep = fmaf(f, o->E32[j1] - o->E32[j], o->E32[j]);
-            float v = fmaf(kappa, Ep, p->vx[i]);
-            p->vx[i] = v;
-            p->x[i] = x + v;
-        }
+        for (int64_t i = 0; i < p->n; ++i) gather_push(o->E32, kappa, Nc, c->bc, &p->x[i], &p->vx[i]);
     }
     /* 2. boundary (L41): electrons first, then ions */
     o->n_abs = 0;
@@ -785,3 +789,151 @@ int oracle_solve_field(int n_cells, int bc, const double* rho, double phi0, doub
     free(o.tmp); free(o.E32);
     return 0;
 }
+
+/* ====================================================================================================
+ * f2 -- the paper's own GAPPED IN-PLACE fine sort (Fig. 2, L63 section 3.2
+ * section 3.7, Fig. 6-9), stated step by step: every sort cell owns n_max slots, the first N_i of them
+ * valid; the free slots at the end serve as the sorting buffer.
+ *   push (fused, L182)  every valid particle is pushed in place
+ *   step 1a (L166)      particles that left their cell are copied to the free slots at the END of the
+ *                       cell (index counted down from n_max); particles that left the box are dropped
+ *   step 1b (L168)      the gaps are closed with the last valid particles of the cell
+ *   step 2  (L184)      cell i takes from the rejected buffers of cells i-1 and i+1 what belongs to i
+ *   step 3  (L186)      rejected particles that moved farther than one cell go straight to their cell
+ * The order inside a cell is undefined in the paper (atomic counters); what IS defined is the result as
+ * a multiset: afterwards cell k holds exactly the surviving particles with key k ("all particles are
+ * arranged in correct sorting cells", L192).  Pin: that multiset, taken from the compact stable sort of
+ * the same particles (sort_species above), tests/test_oracle_gapped.py.  Bounded box only.
+ * ==================================================================================================== */
+typedef struct {
+    int n_cells, n_sc, n_max;
+    float inv_r, kappa;
+    float *x, *vx, *vy, *vz; /* n_sc * n_max slots each */
+    int32_t *N, *R;          /* valid / rejected particles per sort cell */
+    float* E32;              /* n_cells + 1 nodes */
+    uint8_t* hole;           /* scratch: n_max flags */
+    int64_t absorbed_left, absorbed_right, moved_near, moved_far;
+    int error;               /* -2: a cell overflowed (particles dropped) */
+} orc_gapped;
+
+int oracle_gapped_destroy(orc_gapped* g) {
+    if (!g) return 0;
+    free(g->x); free(g->vx); free(g->vy); free(g->vz); free(g->N); free(g->R); free(g->E32); free(g->hole);
+    free(g);
+    return 0;
+}
+
+int oracle_gapped_create(int n_cells, double sort_inv_ratio, int n_max, double kappa, orc_gapped** out) {
+    if (!out || n_cells < 2 || n_max < 1 || !(sort_inv_ratio > 0.0)) return -1;
+    orc_gapped* g = (orc_gapped*)calloc(1, sizeof(orc_gapped));
+    g->n_cells = n_cells; g->n_max = n_max; g->kappa = (float)kappa; g->inv_r = (float)sort_inv_ratio;
+    g->n_sc = (int)ceil((double)n_cells * sort_inv_ratio);
+    size_t tot = (size_t)g->n_sc * (size_t)n_max;
+    g->x = malloc(tot * 4); g->vx = malloc(tot * 4); g->vy = malloc(tot * 4); g->vz = malloc(tot * 4);
+    g->N = calloc((size_t)g->n_sc, 4); g->R = calloc((size_t)g->n_sc, 4);
+    g->E32 = calloc((size_t)n_cells + 2, 4);
+    g->hole = malloc((size_t)n_max);
+    *out = g;
+    return 0;
+}
+
+static int gapped_key(const orc_gapped* g, float x) { /* -1 / -2: left the box (L41) */
+    if (!(x >= 0.0f && x < (float)g->n_cells)) return x < 0.0f ? -1 : -2;
+    return (int)(x * g->inv_r);
+}
+
+static void gapped_put(orc_gapped* g, size_t dst, size_t src) {
+    g->x[dst] = g->x[src]; g->vx[dst] = g->vx[src]; g->vy[dst] = g->vy[src]; g->vz[dst] = g->vz[src];
+}
+
+/* append to cell k behind its valid particles, in front of its rejected buffer */
+static void gapped_append(orc_gapped* g, int k, size_t src) {
+    if (g->N[k] >= g->n_max - g->R[k]) { g->error = -2; return; }
+    gapped_put(g, (size_t)k * g->n_max + (size_t)g->N[k], src);
+    g->N[k]++;
+}
+
+int oracle_gapped_load(orc_gapped* g, int64_t n, const float* x, const float* vx, const float* vy, const float* vz) {
+    if (!g) return -1;
+    memset(g->N, 0, (size_t)g->n_sc * 4); memset(g->R, 0, (size_t)g->n_sc * 4);
+    g->absorbed_left = g->absorbed_right = g->moved_near = g->moved_far = 0; g->error = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        int k = gapped_key(g, x[i]);
+        if (k < 0) return -1;
+        if (g->N[k] >= g->n_max) { g->error = -2; continue; }
+        size_t d = (size_t)k * g->n_max + (size_t)g->N[k]++;
+        g->x[d] = x[i]; g->vx[d] = vx[i]; g->vy[d] = vy[i]; g->vz[d] = vz[i];
+    }
+    return g->error;
+}
+
+int oracle_gapped_set_E32(orc_gapped* g, const float* E32, int n_nodes) {
+    if (!g || n_nodes != g->n_cells + 1) return -1;
+    memcpy(g->E32, E32, (size_t)n_nodes * 4);
+    return 0;
+}
+
+int oracle_gapped_step(orc_gapped* g) {
+    if (!g) return -1;
+    int nm = g->n_max;
+    /* push + step 1a + step 1b, cell by cell */
+    for (int c = 0; c < g->n_sc; ++c) {
+        size_t base = (size_t)c * nm;
+        int N = g->N[c], top = nm, holes = 0;
+        for (int j = 0; j < N; ++j) {
+            gather_push(g->E32, g->kappa, g->n_cells, 0, &g->x[base + j], &g->vx[base + j]);
+            int k = gapped_key(g, g->x[base + j]);
+            g->hole[j] = 0;
+            if (k == c) continue;
+            g->hole[j] = 1; ++holes;
+            if (k == -1) { g->absorbed_left++; continue; }
+            if (k == -2) { g->absorbed_right++; continue; }
+            if (top - 1 < N) { g->error = -2; continue; }       /* no free slot left at the end of the cell */
+            --top;                                               /* step 1a: N_index counts down (L166) */
+            gapped_put(g, base + top, base + j);
+        }
+        int V = N - holes, last = N - 1;                          /* step 1b: close the gaps from the end */
+        for (int j = 0; j < V; ++j) {
+            if (!g->hole[j]) continue;
+            while (g->hole[last]) --last;
+            gapped_put(g, base + j, base + last);
+            --last;
+        }
+        g->N[c] = V; g->R[c] = nm - top;
+    }
+    /* step 2: what the neighbours rejected and belongs here (L184) */
+    for (int c = 0; c < g->n_sc; ++c)
+        for (int d = -1; d <= 1; d += 2) {
+            int nb = c + d;
+            if (nb < 0 || nb >= g->n_sc) continue;
+            size_t nbase = (size_t)nb * nm;
+            for (int q = nm - g->R[nb]; q < nm; ++q)
+                if (gapped_key(g, g->x[nbase + q]) == c) { gapped_append(g, c, nbase + q); g->moved_near++; }
+        }
+    /* step 3: the rare particles that moved farther than one cell (L186) */
+    for (int c = 0; c < g->n_sc; ++c) {
+        size_t base = (size_t)c * nm;
+        for (int q = nm - g->R[c]; q < nm; ++q) {
+            int k = gapped_key(g, g->x[base + q]);
+            if (k == c - 1 || k == c + 1) continue;
+            gapped_append(g, k, base + q); g->moved_far++;
+        }
+    }
+    for (int c = 0; c < g->n_sc; ++c) g->R[c] = 0;               /* the buffers are free again */
+    return g->error;
+}
+
+/* copies the gapped arrays (n_sc * n_max slots) and the counts; stats = {absorbed_left, absorbed_right,
+ * moved_near, moved_far} */
+int oracle_gapped_get(orc_gapped* g, int32_t* N, float* x, float* vx, float* vy, float* vz, int64_t* stats) {
+    if (!g) return -1;
+    size_t tot = (size_t)g->n_sc * (size_t)g->n_max;
+    if (N) memcpy(N, g->N, (size_t)g->n_sc * 4);
+    if (x) memcpy(x, g->x, tot * 4);
+    if (vx) memcpy(vx, g->vx, tot * 4);
+    if (vy) memcpy(vy, g->vy, tot * 4);
+    if (vz) memcpy(vz, g->vz, tot * 4);
+    if (stats) { stats[0] = g->absorbed_left; stats[1] = g->absorbed_right; stats[2] = g->moved_near; stats[3] = g->moved_far; }
+    return g->error;
+}
+int oracle_gapped_n_sort_cells(orc_gapped* g) { return g ? g->n_sc : -1; }
