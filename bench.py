@@ -178,6 +178,54 @@ def read_traffic(kernel):
     return None
 
 
+def gsort_arm(args, p, sim, parts, torch):
+    """push + sort of the ION species (Eq. 5 holds for it in every config) through the paper's
+    gapped in-place sort (include/pic1d_gsort.h) and through the compact count / scan / scatter, same particles,
+    same field, CUDA events; bytes per particle-step beside the times."""
+    from paper_1104_3998_b200 import gsort as GS
+    from paper_1104_3998_b200 import pic1d as G
+    s_ion = 1
+    sim.step(args.warmup)
+    torch.cuda.synchronize()
+    n_ion = sim.moments(s_ion)["count"]
+    agg = {}
+    for _ in range(args.steps):
+        for name, sp, kms in sim.step_timed():
+            if sp == s_ion and name in ("push_count", "bin_scan", "push_scatter"):
+                agg[name] = agg.get(name, 0.0) + kms / args.steps
+    compact_ms = sum(agg.values())
+    E32 = sim.debug_get(G.DBG_E32)
+    x, vx, vy, vz = [sim.debug_get(w, s_ion) for w in (G.DBG_X, G.DBG_VX, G.DBG_VY, G.DBG_VZ)]
+    sim.close()
+    n_max = min(8192, (int(1.5 * p["ppc"] * p["sort_ratio"]) + 255) // 256 * 256)
+    gs = GS.GappedSort(p["n_cells"], p["sort_inv_ratio"], n_max, p["species"][s_ion]["kappa"])
+    gs.load(x, vx, vy, vz)
+    gs.set_E32(E32)
+    gs.step(3)
+    st0 = gs.get(arrays=False)[2]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(gs.stream)
+    gs.step(args.steps)
+    e1.record(gs.stream)
+    torch.cuda.synchronize()
+    N, _, st1 = gs.get(arrays=False)
+    gap_ms = e0.elapsed_time(e1) / args.steps
+    movers = (st1["moved_near"] + st1["moved_far"] - st0["moved_near"] - st0["moved_far"]) / args.steps / max(N.sum(), 1)
+    peak, _ = measured_peak()
+    gap_bytes = (16.0 + 64.0 * movers) * float(N.sum())
+    cmp_bytes = 40.0 * n_ion
+    print(json.dumps({
+        "metric": "push + fine sort of the ion species, ms per step", "workload": workload_name(p), "ions": int(n_ion),
+        "compact": {"ms": compact_ms, "kernels_ms": agg, "bytes_per_particle": 40.0,
+                    "frac_of_peak": cmp_bytes / (compact_ms * 1e-3) / 1e9 / peak},
+        "gapped": {"ms": gap_ms, "n_max": n_max, "movers_per_step": movers, "error": st1["error"],
+                   "bytes_per_particle": 16.0 + 64.0 * movers,
+                   "frac_of_peak": gap_bytes / (gap_ms * 1e-3) / 1e9 / peak,
+                   "note": "in-place push 16 B per particle + 64 B per mover (buffer write + read + final write, 4 arrays)"},
+        "speedup_gapped_over_compact": compact_ms / gap_ms}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -198,6 +246,8 @@ def main():
     ap.add_argument("--no-graph", action="store_true", help="no CUDA graph replay in pic1d_step")
     ap.add_argument("--mcc-gather", action="store_true", help="k_mcc without the bulk-copy staging of velocities")
     ap.add_argument("--fold-all", action="store_true", help="fold the collisions of every species into its scatter")
+    ap.add_argument("--gsort", action="store_true",
+                    help="f2: time the paper's gapped in-place push + sort on the ions beside the compact sort")
     ap.add_argument("--profile", action="store_true",
                     help="timed region only (no per-kernel pass, e2e or CPU baseline): the command ncu wraps")
     args = ap.parse_args()
@@ -248,6 +298,9 @@ def main():
 
     def live():
         return [sim.moments(s) for s in range(ns)]
+
+    if args.gsort:
+        return gsort_arm(args, p, sim, parts, torch)
 
     sim.step(args.warmup)
     barrier()
