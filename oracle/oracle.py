@@ -20,11 +20,16 @@ _DTYPES = {X: np.float32, VX: np.float32, VY: np.float32, VZ: np.float32, KEYS: 
            OFFSETS: np.int32, MASK: np.uint8, E32: np.float32, RHO_S: np.float64, PARTNER: np.int32}
 
 
+_EXTRA = os.environ.get("ORACLE_CFLAGS", "").split()  # e.g. -fsanitize=address,undefined -g (profiles/r2_sanitizers.md)
+if _EXTRA:
+    _LIB = os.path.join(_HERE, "libpic1d_oracle_san.so")   # an instrumented build never replaces the plain one
+
+
 def build(force=False):
     """gcc -O2 -ffp-contract=off: every fp32 op is the IEEE op that is written."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math",
-                               "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math"] + _EXTRA +
+                              ["-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
     return _LIB
 
 
