@@ -382,7 +382,8 @@ def main():
     roofline = {"bound": "hbm", "kernel": dom_name,
                 "achieved": dom["alg_GBps"], "peak": peak, "unit": "GB/s", "frac": dom["alg_GBps"] / peak,
                 "traffic": None, "peak_source": peak_src, "alg_bytes_per_launch": dom["alg_bytes"],
-                "kernel_ms": dom["ms"], "particles_per_launch": stat[dom["species"]][0],
+                "kernel_ms": dom["ms"],
+                "particles_per_launch": stat[dom["species"]][0] if dom["species"] >= 0 else sum(stat[q][0] for q in range(ns)),
                 "step": {"as_built": {"bytes_per_particle": step_bytes / n_live, "alg_bytes": step_bytes,
                                       "achieved": step_bytes / step_s / 1e9, "frac": step_bytes / step_s / 1e9 / peak,
                                       "frac_of_8TBps": step_bytes / step_s / 1e9 / 8000.0,
