@@ -148,8 +148,8 @@ def algorithmic_bytes(name, n_src, n_out, cand_frac, coll_frac, folded):
         return 8.0 * n_src                       # read x, vx
     if name == "push_scatter":
         return 16.0 * n_src + 16.0 * n_out       # read 4 arrays, write 4 arrays (folded MCC: nothing more)
-    if name == "bin_scan" and folded:
-        return n_src / 8.0                       # null-test bit mask written (read again by the scatter: L2)
+    if name == "null_bits":
+        return n_src / 8.0                       # next step's null-test bit mask written (read by its scatter: L2)
     if name == "deposit":
         return 4.0 * n_out                       # read sorted x
     if name == "mcc":
@@ -387,7 +387,7 @@ def main():
                 "step": {"as_built": {"bytes_per_particle": step_bytes / n_live, "alg_bytes": step_bytes,
                                       "achieved": step_bytes / step_s / 1e9, "frac": step_bytes / step_s / 1e9 / peak,
                                       "frac_of_8TBps": step_bytes / step_s / 1e9 / 8000.0,
-                                      "pipeline": "count 8 + scatter 32 + deposit 4 = 44 B + MCC (own pass: sectors touched; folded: 1/8 B bit mask)"},
+                                      "pipeline": "count 8 + scatter 32 + deposit 4 = 44 B + MCC (own pass: sectors touched; folded: 1/8 B bit mask, computed one step ahead)"},
                          "canonical_52B": {"bytes_per_particle": canon / n_live, "alg_bytes": canon,
                                            "achieved": canon / step_s / 1e9, "frac": canon / step_s / 1e9 / peak,
                                            "frac_of_8TBps": canon / step_s / 1e9 / 8000.0,

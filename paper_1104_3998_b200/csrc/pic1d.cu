@@ -75,6 +75,7 @@ struct pic1d {
     void (*k_scatter[2][2])(SortArgs);  // [species][0 plain | 1 the step's, with the MCC folded in]
     cudaStream_t side;              // collisions run here beside the deposit and the field solve
     cudaEvent_t ev_fork, ev_join;
+    bool null_ready;                // the null-test masks of the NEXT step have been enqueued (by the previous step)
     cudaGraphExec_t graph[2];       // two captured steps, per parity of the sort buffers at their start
     int64_t launches_per_2steps;
     bool timing;
@@ -352,8 +353,8 @@ void enqueue_sort(pic1d* h, int s, int in_step, int shift = 0) {
     h->k_count[s]<<<gc, PIC1D_NT, h->smem_count[s], h->stream>>>(a);
     mark(h, "push_count", s);
     const bool fold = in_step && p.mcck;
-    a.null_first = a.abs_list ? 1 : 0;
-    const int nb_null = fold ? (p.capacity / 32 + BINSCAN_NW * 32 - 1) / (BINSCAN_NW * 32) : 0;
+    a.null_first = a.abs_list ? PIC1D_DEAD_CHUNKS : 0;  // blocks that scan the per-tile absorbed counts
+    const int nb_null = (fold && !h->null_ready) ? (p.capacity / 32 + BINSCAN_NW * 32 - 1) / (BINSCAN_NW * 32) : 0;
     k_bin_scan<<<(a.n_sc + 31) / 32 + a.null_first + nb_null, BINSCAN_NW * 32, 0, h->stream>>>(a);
     mark(h, "bin_scan", s);
     h->k_scatter[s][in_step]<<<gs, PIC1D_NT, h->smem_scatter[s], h->stream>>>(a);
@@ -460,8 +461,19 @@ void enqueue_mcc(pic1d* h, cudaStream_t st) {
     }
 }
 
+// the null-test bit mask of species s for the NEXT step (k_null_bits_next), once this step's scatter has used the
+// current one.  Placement measured (profiles/r2_notes.md): at the end of the side stream's work, after the births.
+void enqueue_null_next(pic1d* h, int s, cudaStream_t st) {
+    SpeciesHost& p = h->sp[s];
+    if (!p.mcck) return;
+    const int n_words = p.capacity / 32;
+    k_null_bits_next<<<(n_words + 255) / 256, 256, 0, st>>>(mcc_params(h, s), n_words);
+    mark(h, "null_bits", s);
+}
+
 void enqueue_step(pic1d* h) {
     const pic1d_config_t& c = h->cfg;
+    const bool overlap = h->side != nullptr && !h->timing && !(c.flags & PIC1D_FLAG_NO_OVERLAP);
     enqueue_begin(h, 1);
     if (c.n_species > 1) {
         enqueue_sort(h, 1, 1);
@@ -479,19 +491,21 @@ void enqueue_step(pic1d* h) {
     }
     enqueue_sort(h, 0, 1);
     // fork: collisions + births on the side stream, deposit + field on the caller's; join at the end of the step
-    const bool overlap = h->side != nullptr && !h->timing && !(c.flags & PIC1D_FLAG_NO_OVERLAP);
     if (overlap) {
         cudaEventRecord(h->ev_fork, h->stream);
         cudaStreamWaitEvent(h->side, h->ev_fork, 0);
         enqueue_mcc(h, h->side);
+        for (int s = c.n_species - 1; s >= 0; --s) enqueue_null_next(h, s, h->side);
         cudaEventRecord(h->ev_join, h->side);
         enqueue_grid(h, 1);
         cudaStreamWaitEvent(h->stream, h->ev_join, 0);
     } else {
         enqueue_grid(h, 1);
         enqueue_mcc(h, h->stream);
+        for (int s = c.n_species - 1; s >= 0; --s) enqueue_null_next(h, s, h->stream);
     }
     h->step += 1u;
+    h->null_ready = true;
 }
 
 int sticky_code(unsigned err) {
@@ -588,6 +602,7 @@ int pic1d_load_particles(pic1d_t* h, int s, int64_t n, const float* x, const flo
     if (n > p.capacity) return PIC1D_ERR_CAPACITY;
     if (h->loaded_mask == 0) {  // a new run starts: all species must be (re)loaded
         h->ready = false;
+        h->null_ready = false;
         for (int q = 0; q < h->cfg.n_species; ++q) h->sp[q].cur = 0;
         k_clear_err<<<1, 1, 0, h->stream>>>(h->st);
         h->launches++;
@@ -648,6 +663,7 @@ int pic1d_step(pic1d_t* h, int n_steps) {
     // Two consecutive steps (the sort buffers swap every step, so two steps restore the pointers) are captured
     // once per buffer parity into a CUDA graph and replayed: every per-step quantity (step index, particle
     // counts, tickets) lives in DevState on the device, no kernel argument changes from step to step.
+    if (!h->null_ready && n_steps > 0) { enqueue_step(h); k = 1; }  // (a captured step counts on the masks computed ahead)
     if (!(h->cfg.flags & PIC1D_FLAG_NO_GRAPH)) {
         while (n_steps - k >= 2) {
             const int par = h->sp[0].cur;
@@ -813,7 +829,7 @@ int pic1d_debug_set_state(pic1d_t* h, int s, int64_t n, int64_t n_sorted, const 
         if (!src[k] || !ck(h, cudaMemcpyAsync(p.buf[p.cur][k], src[k], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, h->stream)))
             return PIC1D_ERR_CUDA;
     k_debug_set_counts<<<1, 1, 0, h->stream>>>(h->st, s, (int)n, (int)n_sorted, step >= 0 ? 1 : 0, (unsigned)(step >= 0 ? step : 0));
-    if (step >= 0) h->step = (uint32_t)step;
+    if (step >= 0) { h->step = (uint32_t)step; h->null_ready = false; }  // the masks enqueued ahead belong to another step index
     return ck(h, cudaStreamSynchronize(h->stream)) ? PIC1D_OK : PIC1D_ERR_CUDA;
 }
 

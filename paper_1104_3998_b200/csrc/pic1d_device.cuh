@@ -10,6 +10,7 @@
 #define PIC1D_NWARP (PIC1D_NT / 32)
 #define PIC1D_WA_MAX 1920     // bins of a tile window ranked at a time in shared memory (multiple of 8)
 #define PIC1D_GROUP 64        // tiles per tile-group (window union used by the bin scan)
+#define PIC1D_DEAD_CHUNKS 64  // blocks that scan the per-tile absorbed counts (see DevSpecies)
 
 // Philox stream ids (R12)
 #define STREAM_NULL 0u
@@ -41,6 +42,10 @@ struct DevSpecies {
     int scan_done; // bin blocks of k_bin_scan that have finished (the last one scans the histogram)
     ull absorbed_left, absorbed_right, injected, n_candidates, n_events[4], births, dropped, over_cap;
     ull reflected, n_pairs;  // f4: electrons reflected at a wall; f3: binary collisions performed
+    // ordered absorbed list (ions with secondary emission): the per-tile absorbed counts are scanned in
+    // PIC1D_DEAD_CHUNKS chunks by as many blocks; the block that finishes last turns the chunk totals into bases
+    int dead_done;
+    int dead_tot[PIC1D_DEAD_CHUNKS], dead_base[PIC1D_DEAD_CHUNKS];
 };
 
 struct DevState {
@@ -82,6 +87,11 @@ __device__ __forceinline__ int atom_shared_add(int* p, int v) {
     const unsigned a = (unsigned)__cvta_generic_to_shared(p);
     asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(a), "r"(v) : "memory");
     return old;
+}
+
+// tiles per chunk of the absorbed-count scan (a multiple of 32); the same on both sides of the scan
+__device__ __forceinline__ int dead_chunk_tiles(int n_tiles) {
+    return ((n_tiles + PIC1D_DEAD_CHUNKS - 1) / PIC1D_DEAD_CHUNKS + 31) & ~31;
 }
 
 __device__ __forceinline__ int warp_min(int v) {

@@ -205,6 +205,25 @@ __device__ __forceinline__ void mcc_null_words(const MccP& m, int wd) {
     m.null_bits[wd] = m.null_any ? bits : 0u;
 }
 
+// The same mask one step AHEAD: the null test of slot d depends on (seed, step, species, d) only, so the mask of step
+// n + 1 is computed while step n's electron sort runs (side stream; that kernel leaves most issue slots idle) and
+// the extra blocks of k_bin_scan are not needed.  All capacity / 32 words: the next step's particle count is not
+// known yet (births, secondaries).
+__global__ void __launch_bounds__(256) k_null_bits_next(MccP m, int n_words) {
+    const int wd = blockIdx.x * blockDim.x + threadIdx.x;
+    if (wd >= n_words) return;
+    const uint32_t step = m.st->step_next;
+    unsigned bits = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        uint32_t w[4];
+        philox4x32_10((uint32_t)(wd * 8 + q), step, STREAM_NULL + (uint32_t)m.s, 0u, m.k0, m.k1, w);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) bits |= (w[c] <= m.null_le ? 1u : 0u) << (4 * q + c);
+    }
+    m.null_bits[wd] = m.null_any ? bits : 0u;
+}
+
 // warp-reduce the packed per-thread counters and add them to the species' cumulative counters
 __device__ __forceinline__ void mcc_flush_counts(const MccP& m, const MccCount& c) {
     int vals[5] = {(int)(c.cand_e1 & 0xffffu), (int)(c.cand_e1 >> 16), (int)(c.e2_e3 & 0xffffu), (int)(c.e2_e3 >> 16), (int)c.over};

@@ -280,7 +280,8 @@ __device__ void bin_scan_finish(const SortArgs& a) {
     }
 }
 
-#define BINSCAN_NW 32
+#define BINSCAN_NW 16  // warps per block; with 16 tiles in flight per warp the best of the sweep in profiles/r2_notes.md
+#define BINSCAN_B 16   // tiles in flight per warp
 #define BINSCAN_LIST 4096
 #define BINSCAN_DESC 2048  // tile descriptors a block can keep in shared memory
 __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
@@ -297,11 +298,30 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
         return;
     }
     if ((int)blockIdx.x >= nb_bins) {
-        // one extra block (species with an ordered absorbed list only): exclusive prefix of the per-tile
-        // absorbed counts, concurrently with the bin blocks
+        // PIC1D_DEAD_CHUNKS extra blocks (species with an ordered absorbed list only), concurrently with the bin
+        // blocks: exclusive prefix of the per-tile absorbed counts inside the block's chunk of tiles; the block
+        // that finishes last turns the chunk totals into chunk bases (the scatter adds base + prefix).  One block
+        // scanning all 2.7e5 warp tiles of config 4 took 70 us and bounded the whole launch.
+        __shared__ int s_last_dead;
         DevSpecies& sp = a.st->sp[a.s];
-        const int n_dead = block_exclusive_scan<true>(a.tile_dead, a.tile_dead, sp.n_tiles);
-        if (tid == 0) sp.n_dead = n_dead;
+        const int c = (int)blockIdx.x - nb_bins, ch = dead_chunk_tiles(sp.n_tiles);
+        const int b = min(c * ch, sp.n_tiles), e = min(b + ch, sp.n_tiles);
+        const int tot = block_exclusive_scan<true>(a.tile_dead + b, a.tile_dead + b, e - b);
+        if (tid == 0) {
+            sp.dead_tot[c] = tot;
+            __threadfence();
+            s_last_dead = atomicAdd(&sp.dead_done, 1) == PIC1D_DEAD_CHUNKS - 1;
+        }
+        __syncthreads();
+        if (s_last_dead && tid == 0) {
+            __threadfence();
+            int run = 0;
+            for (int q = 0; q < PIC1D_DEAD_CHUNKS; ++q) {
+                sp.dead_base[q] = run;
+                run += *reinterpret_cast<volatile int*>(&sp.dead_tot[q]);
+            }
+            sp.n_dead = run;
+        }
         return;
     }
     const int kb0 = blockIdx.x * 32, kb1 = min(kb0 + 31, a.n_sc - 1);
@@ -340,7 +360,7 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
     const int n_virt = (listed ? n_rel : n_groups) * PIC1D_GROUP;
     const int chunk = (n_virt + BINSCAN_NW - 1) / BINSCAN_NW;
     const int v_beg = min(wp * chunk, n_virt), v_end = min(v_beg + chunk, n_virt);
-    constexpr int B = 8;  // tiles in flight per warp: the loads of a batch are independent
+    constexpr int B = BINSCAN_B;  // tiles in flight per warp: the loads of a batch are independent
     if (listed && n_virt <= BINSCAN_DESC) {
         // usual case: the descriptors (lo, w, off) of the listed tiles are fetched once, coalesced, into
         // shared memory; both passes then read them with one broadcast LDS.128 and no index arithmetic
@@ -374,22 +394,22 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
             total += v;
         }
         for (int v0 = v_beg; v0 < v_end; v0 += B) {
-            int* p[B];
+            int p[B];  // index into the pool, -1: the tile's window does not hold the cell
             int c[B];
 #pragma unroll
             for (int b = 0; b < B; ++b) {
-                p[b] = nullptr;
+                p[b] = -1;
                 c[b] = 0;
                 if (v0 + b < v_end) {
                     const int4 d = s_desc[v0 + b];
                     const unsigned r = (unsigned)(k - d.x);
-                    if (r < (unsigned)d.y) p[b] = a.pool + d.z + r;
+                    if (r < (unsigned)d.y) p[b] = d.z + (int)r;
                 }
             }
 #pragma unroll
-            for (int b = 0; b < B; ++b) if (p[b]) c[b] = __ldcg(p[b]);
+            for (int b = 0; b < B; ++b) if (p[b] >= 0) c[b] = __ldcg(a.pool + p[b]);
 #pragma unroll
-            for (int b = 0; b < B; ++b) if (p[b]) { __stcg(p[b], run); run += c[b]; }
+            for (int b = 0; b < B; ++b) if (p[b] >= 0) { __stcg(a.pool + p[b], run); run += c[b]; }
         }
         if (wp == 0 && k < a.n_sc) a.hist[k] = total;
         bin_scan_finish(a);
@@ -750,6 +770,7 @@ __global__ void k_step_begin(BeginArgs b) {
             sp.ticket = 0;
             sp.ticket2 = 0;
             sp.scan_done = 0;
+            sp.dead_done = 0;
         }
         st->n_abs = 0;
         if (b.mode) { st->step = st->step_next; st->step_next = st->step + 1u; }

@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_push_scatter_w(SortArgs a) {
         unsigned c0 = 0;
         if (narrow && lane < w) c0 = (unsigned)(a.offsets[lo + lane] + __ldcg(a.pool + off + lane));
         unsigned cdead = 0;
-        if (ABS) cdead = (unsigned)a.tile_dead[tile];
+        if (ABS) cdead = (unsigned)a.tile_dead[tile];  // prefix inside the tile's chunk of the absorbed-count scan
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
             const int i = base + r * 32;
@@ -192,6 +192,12 @@ __global__ void __launch_bounds__(PIC1D_NT, 4) k_push_scatter_w(SortArgs a) {
                 k[r] = key >= 0 ? key - lo : (ABS ? w : -1);
                 if (ABS && key == -2) wall |= 1u << r;
             }
+        }
+        if (ABS) {  // rare: the tile lost particles to a wall -> its place in the ordered absorbed list needs the chunk's base
+            bool dead = false;
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) dead |= k[r] == w;
+            if (__any_sync(0xffffffffu, dead)) cdead += (unsigned)sp.dead_base[tile / dead_chunk_tiles(n_tiles)];
         }
         if (full) {
 #pragma unroll
