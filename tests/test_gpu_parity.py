@@ -500,6 +500,33 @@ def test_scheduling_variants_give_identical_results():
             assert np.array_equal(a, b)
 
 
+@pytest.mark.parametrize("mcc", ["folded", "own_pass"])
+def test_resume_at_another_step_index(mcc):
+    """pic1d_debug_set_state with a step index: the run continues at step n of the oracle although the GPU handle
+    itself is at step 2 -- every Philox stream is keyed on the step, and the null-test masks the library computes
+    one step ahead (k_null_bits_next) belong to the old index and must be recomputed"""
+    from oracle import oracle as O
+    from paper_1104_3998_b200 import pic1d as G
+    o, g, p = _mk(dict(W.make_params(2, n_cells=256, ppc=150), no_fold=(mcc == "own_pass")))
+    assert o.step(6) == 0
+    g.step(2)
+    for jump in (6, 7):
+        for s in range(p["n_species"]):
+            g.set_state(s, o.moments(s)["n_sorted"], *[o.debug_get(w, s) for w in (O.X, O.VX, O.VY, O.VZ)], step=jump)
+        g.set_E32(o.debug_get(O.E32))
+        assert o.step(1) == 0
+        g.step(1)
+        assert g.step_index == jump + 1
+        for s in range(p["n_species"]):
+            assert np.array_equal(o.debug_get(O.OFFSETS, s), g.debug_get(G.DBG_OFFSETS, s))
+            assert np.array_equal(o.debug_get(O.KEYS, s), g.debug_get(G.DBG_KEYS, s))
+            assert np.array_equal(o.debug_get(O.MASK, s), g.debug_get(G.DBG_MASK, s)) and o.debug_get(O.MASK, s).any()
+            assert np.array_equal(o.debug_get(O.X, s), g.debug_get(G.DBG_X, s))
+            assert _vel_err([g.debug_get(w, s) for w in (G.DBG_VX, G.DBG_VY, G.DBG_VZ)],
+                            [o.debug_get(w, s) for w in (O.VX, O.VY, O.VZ)]) <= TOL_V
+    o.close(); g.close()
+
+
 def test_moments_and_eedf_bit_for_bit():
     """pic1d_moments with an EEDF histogram (n_bins > 0) against oracle_moments: the histogram bit for bit (both
     bin E = c_eV |v|^2 in fp64 with the same operations), the sums to fp64 rounding"""
