@@ -315,7 +315,7 @@ void setup_launch(pic1d* h) {
     cudaFuncSetAttribute(k_mcc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     h->WA = std::min((h->n_sc + 1 + 7) / 8 * 8, PIC1D_WA_MAX);
-    h->smem_sort = (size_t)h->WA * sizeof(int);
+    h->smem_sort = (size_t)(h->WA + 1) * sizeof(int);
     for (int s = 0; s < h->cfg.n_species; ++s) {
         SpeciesHost& p = h->sp[s];
         const bool abs = s == 1 && h->abs_list != nullptr;

@@ -56,7 +56,7 @@ struct SortArgs {
 // the position in the pool carries no meaning, so this atomic decides no particle index.
 template <int BC, int V>
 __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
-    extern __shared__ int s_hist[];  // WA counters, all zero between tiles
+    extern __shared__ int s_hist[];  // WA counters, all zero between tiles (+ one slot for keys outside the sub-window)
     __shared__ int s_lohi[2][2];     // block min / max of the keys, double-buffered over tiles
     __shared__ int s_dead[2][2];     // absorbed left / right, double-buffered
     __shared__ int s_off;
@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count(SortArgs a) {
 #pragma unroll
             for (int q = 0; q < 4 * V; ++q) {
                 const unsigned r = (unsigned)(keys[q] - klo);
-                if (r < (unsigned)nsub) atomicAdd(&s_hist[r], 1);
+                atomicAdd(&s_hist[r < (unsigned)nsub ? r : (unsigned)WA], 1);  // branch-free: slot WA swallows the rest (never read)
             }
             __syncthreads();
             for (int i = tid; i < nsub; i += PIC1D_NT) {

@@ -23,7 +23,7 @@
 
 template <int BC>
 __global__ void __launch_bounds__(PIC1D_NT) k_push_count_w(SortArgs a) {
-    __shared__ int s_h[PIC1D_NWARP][PIC1D_PSW];
+    __shared__ int s_h[PIC1D_NWARP][PIC1D_PSW + 1];  // + a slot that swallows the keys outside the window (never read)
     const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
     DevSpecies& sp = a.st->sp[a.s];
     const int n_tiles = sp.n_tiles, n_src = sp.n_src, n_push = sp.n_push;
@@ -123,8 +123,8 @@ __global__ void __launch_bounds__(PIC1D_NT) k_push_count_w(SortArgs a) {
             __syncwarp();
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-                const unsigned r = (unsigned)(keys[q] - lo);
-                if (r < (unsigned)PIC1D_PSW) atomicAdd(&s_h[wp][r], 1);
+                const unsigned r = (unsigned)(keys[q] - lo);  // absorbed: huge
+                atomicAdd(&s_h[wp][min(r, (unsigned)PIC1D_PSW)], 1);  // branch-free
             }
             __syncwarp();
             if (lane < w) a.pool[off + lane] = s_h[wp][lane];
