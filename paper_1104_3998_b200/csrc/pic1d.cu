@@ -829,7 +829,8 @@ int pic1d_debug_set_state(pic1d_t* h, int s, int64_t n, int64_t n_sorted, const 
         if (!src[k] || !ck(h, cudaMemcpyAsync(p.buf[p.cur][k], src[k], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, h->stream)))
             return PIC1D_ERR_CUDA;
     k_debug_set_counts<<<1, 1, 0, h->stream>>>(h->st, s, (int)n, (int)n_sorted, step >= 0 ? 1 : 0, (unsigned)(step >= 0 ? step : 0));
-    if (step >= 0) { h->step = (uint32_t)step; h->null_ready = false; }  // the masks enqueued ahead belong to another step index
+    if (step >= 0) h->step = (uint32_t)step;
+    h->null_ready = false;  // the masks enqueued ahead belong to another step index / another particle count
     return ck(h, cudaStreamSynchronize(h->stream)) ? PIC1D_OK : PIC1D_ERR_CUDA;
 }
 

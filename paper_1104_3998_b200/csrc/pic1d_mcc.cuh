@@ -207,10 +207,11 @@ __device__ __forceinline__ void mcc_null_words(const MccP& m, int wd) {
 
 // The same mask one step AHEAD: the null test of slot d depends on (seed, step, species, d) only, so the mask of step
 // n + 1 is computed while step n's electron sort runs (side stream; that kernel leaves most issue slots idle) and
-// the extra blocks of k_bin_scan are not needed.  All capacity / 32 words: the next step's particle count is not
-// known yet (births, secondaries).
+// the extra blocks of k_bin_scan are not needed.  It runs after the births, so the species' n_live is the next step's
+// source count -- except for electrons, which may still receive secondaries: all capacity / 32 words for them.
 __global__ void __launch_bounds__(256) k_null_bits_next(MccP m, int n_words) {
     const int wd = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m.s != 0) n_words = min(n_words, (m.st->sp[m.s].n_live + 31) >> 5);
     if (wd >= n_words) return;
     const uint32_t step = m.st->step_next;
     unsigned bits = 0;
