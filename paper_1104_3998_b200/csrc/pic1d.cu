@@ -354,8 +354,11 @@ void enqueue_sort(pic1d* h, int s, int in_step, int shift = 0) {
     mark(h, "push_count", s);
     const bool fold = in_step && p.mcck;
     a.null_first = a.abs_list ? PIC1D_DEAD_CHUNKS : 0;  // blocks that scan the per-tile absorbed counts
-    const int nb_null = (fold && !h->null_ready) ? (p.capacity / 32 + BINSCAN_NW * 32 - 1) / (BINSCAN_NW * 32) : 0;
-    k_bin_scan<<<(a.n_sc + 31) / 32 + a.null_first + nb_null, BINSCAN_NW * 32, 0, h->stream>>>(a);
+    const int nb_bins = (a.n_sc + 31) / 32;
+    const int nw = (nb_bins < h->num_sms && p.n_tiles_max >= 4096) ? 32 : 16;  // warps per block (see k_bin_scan)
+    const int nb_null = (fold && !h->null_ready) ? (p.capacity / 32 + nw * 32 - 1) / (nw * 32) : 0;
+    if (nw == 16) k_bin_scan<16><<<nb_bins + a.null_first + nb_null, 16 * 32, 0, h->stream>>>(a);
+    else k_bin_scan<32><<<nb_bins + a.null_first + nb_null, 32 * 32, 0, h->stream>>>(a);
     mark(h, "bin_scan", s);
     h->k_scatter[s][in_step]<<<gs, PIC1D_NT, h->smem_scatter[s], h->stream>>>(a);
     mark(h, "push_scatter", s);

@@ -280,21 +280,24 @@ __device__ void bin_scan_finish(const SortArgs& a) {
     }
 }
 
-#define BINSCAN_NW 16  // warps per block; with 16 tiles in flight per warp the best of the sweep in profiles/r2_notes.md
+// NW warps per block: 16 (with 16 tiles in flight per warp the best of the sweep in profiles/r2_notes.md) when the bin
+// blocks alone fill the GPU or the problem is small, 32 when few bin blocks walk many tiles (coarse sort cells: 8
+// blocks for config 3 at r = 16)
 #define BINSCAN_B 16   // tiles in flight per warp
 #define BINSCAN_LIST 4096
 #define BINSCAN_DESC 2048  // tile descriptors a block can keep in shared memory
-__global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
-    __shared__ int s_wc[BINSCAN_NW];
+template <int NW>
+__global__ void __launch_bounds__(NW * 32) k_bin_scan(SortArgs a) {
+    __shared__ int s_wc[NW];
     __shared__ unsigned short s_list[BINSCAN_LIST];  // tile groups whose window overlaps the block's cells
-    __shared__ int s_part[BINSCAN_NW][33];
+    __shared__ int s_part[NW][33];
     __shared__ int4 s_desc[BINSCAN_DESC];
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
     const int nb_bins = (a.n_sc + 31) / 32;
     if ((int)blockIdx.x >= nb_bins + a.null_first) {
         // extra blocks (species whose MCC is folded into the scatter): the null-test bit mask of this step,
         // 1024 words = 32768 slots per block, concurrently with the bin blocks
-        mcc_null_words(a.m, ((int)blockIdx.x - nb_bins - a.null_first) * (BINSCAN_NW * 32) + tid);
+        mcc_null_words(a.m, ((int)blockIdx.x - nb_bins - a.null_first) * (NW * 32) + tid);
         return;
     }
     if ((int)blockIdx.x >= nb_bins) {
@@ -333,7 +336,7 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
     // contiguous chunk of groups [t gpt, (t+1) gpt): count, block-wide exclusive scan, write.
     int n_rel = 0;
     {
-        const int gpt = (n_groups + BINSCAN_NW * 32 - 1) / (BINSCAN_NW * 32);
+        const int gpt = (n_groups + NW * 32 - 1) / (NW * 32);
         const int g_beg = min(tid * gpt, n_groups), g_end = min(g_beg + gpt, n_groups);
         int mine = 0;
         for (int g = g_beg; g < g_end; ++g) mine += (a.grp_hi[g] >= kb0 && a.grp_lo[g] <= kb1) ? 1 : 0;
@@ -347,7 +350,7 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
         __syncthreads();
         int before = 0;
 #pragma unroll 8
-        for (int q = 0; q < BINSCAN_NW; ++q) { const int v = s_wc[q]; if (q < wp) before += v; n_rel += v; }
+        for (int q = 0; q < NW; ++q) { const int v = s_wc[q]; if (q < wp) before += v; n_rel += v; }
         int idx = before + inc - mine;
         if (mine) {
             for (int g = g_beg; g < g_end; ++g)
@@ -358,13 +361,13 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
     // n_rel groups (or, if the list overflowed, every group) -> virtual tile range split over the warps
     const bool listed = n_rel <= BINSCAN_LIST && n_groups <= 65536;
     const int n_virt = (listed ? n_rel : n_groups) * PIC1D_GROUP;
-    const int chunk = (n_virt + BINSCAN_NW - 1) / BINSCAN_NW;
+    const int chunk = (n_virt + NW - 1) / NW;
     const int v_beg = min(wp * chunk, n_virt), v_end = min(v_beg + chunk, n_virt);
     constexpr int B = BINSCAN_B;  // tiles in flight per warp: the loads of a batch are independent
     if (listed && n_virt <= BINSCAN_DESC) {
         // usual case: the descriptors (lo, w, off) of the listed tiles are fetched once, coalesced, into
         // shared memory; both passes then read them with one broadcast LDS.128 and no index arithmetic
-        for (int v = tid; v < n_virt; v += BINSCAN_NW * 32) {
+        for (int v = tid; v < n_virt; v += NW * 32) {
             const int t = (int)s_list[v / PIC1D_GROUP] * PIC1D_GROUP + v % PIC1D_GROUP;
             s_desc[v] = t < n_tiles ? make_int4(a.tile_lo[t], a.tile_w[t], a.tile_off[t], 0) : make_int4(0, 0, 0, 0);
         }
@@ -388,7 +391,7 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
         __syncthreads();
         int run = 0, total = 0;
 #pragma unroll 8
-        for (int q = 0; q < BINSCAN_NW; ++q) {
+        for (int q = 0; q < NW; ++q) {
             const int v = s_part[q][lane];
             if (q < wp) run += v;
             total += v;
@@ -437,7 +440,7 @@ __global__ void __launch_bounds__(BINSCAN_NW * 32) k_bin_scan(SortArgs a) {
     __syncthreads();
     int run = 0, total = 0;
 #pragma unroll 8
-    for (int q = 0; q < BINSCAN_NW; ++q) {
+    for (int q = 0; q < NW; ++q) {
         const int v = s_part[q][lane];
         if (q < wp) run += v;
         total += v;
