@@ -230,11 +230,11 @@ __device__ __forceinline__ void mcc_flush_counts(const MccP& m, const MccCount& 
     int vals[5] = {(int)(c.cand_e1 & 0xffffu), (int)(c.cand_e1 >> 16), (int)(c.e2_e3 & 0xffffu), (int)(c.e2_e3 >> 16), (int)c.over};
 #pragma unroll
     for (int q = 0; q < 5; ++q) vals[q] = __reduce_add_sync(0xffffffffu, vals[q]);
-    if ((threadIdx.x & 31) == 0 && vals[0]) {
+    if ((threadIdx.x & 31) == 0 && (vals[0] | vals[1] | vals[2] | vals[3] | vals[4])) {
         DevSpecies& sp = m.st->sp[m.s];
-        atomicAdd(&sp.n_candidates, (ull)vals[0]);
-        const int nulls = vals[0] - vals[1] - vals[2] - vals[3];
-        if (nulls) atomicAdd(&sp.n_events[0], (ull)nulls);
+        if (vals[0]) atomicAdd(&sp.n_candidates, (ull)vals[0]);
+        const int nulls = vals[0] - vals[1] - vals[2] - vals[3];  // may be negative when the candidates are added elsewhere
+        if (nulls) atomicAdd(&sp.n_events[0], (ull)(long long)nulls);
 #pragma unroll
         for (int q = 1; q < 4; ++q) if (vals[q]) atomicAdd(&sp.n_events[q], (ull)vals[q]);
         if (vals[4]) atomicAdd(&sp.over_cap, (ull)vals[4]);
@@ -299,6 +299,7 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
     const uint32_t step = st->step;
     const uint32_t str_null = STREAM_NULL + (uint32_t)m.s, str_coll = STREAM_COLL + (uint32_t)m.s;
     MccCount cnt = {0u, 0u, 0u};
+    ull n_cand_block = 0;  // thread 0: candidates of the block's tiles (the list lengths)
     unsigned parity = 0;
     if (STAGE && tid == 0) mbar_init(&s_bar, 1);
     while (true) {
@@ -370,10 +371,7 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
                 philox4x32_10((uint32_t)i, step, str_coll, 0u, m.k0, m.k1, b0);
                 bool over;
                 e = mcc_select<KIND>(m, vx, vy, vz, u01(b0[0]), over);
-                cnt.cand_e1 += 1u + (e == 1 ? 0x10000u : 0u);
-                cnt.e2_e3 += (e == 2 ? 1u : 0u) + (e == 3 ? 0x10000u : 0u);
-                cnt.over += over ? 1u : 0u;
-                if (m.mask && e) m.mask[i] = (uint8_t)e;
+                cnt.over += over ? 1u : 0u;  // (the events are counted by phase C, the candidates per tile)
             }
             const int idx = warp_append(e != 0, &s_n[1]);
             if (e) s_coll[idx] = (unsigned short)(rel | (e << 12));
@@ -381,9 +379,13 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
         __syncthreads();
         // ---- phase C: kinematics, one thread per real collision -------------------------------------
         const int n_coll = s_n[1];
+        if (tid == 0) n_cand_block += (ull)n_cand;
         for (int j = tid; j < n_coll; j += PIC1D_NT) {
             const int rel = s_coll[j] & 0xfff, e = s_coll[j] >> 12;
             const int i = tbase + rel;
+            cnt.cand_e1 += e == 1 ? 0x10000u : 0u;
+            cnt.e2_e3 += (e == 2 ? 1u : 0u) + (e == 3 ? 0x10000u : 0u);
+            if (m.mask) m.mask[i] = (uint8_t)e;
             uint32_t b0[4];
             philox4x32_10((uint32_t)i, step, str_coll, 0u, m.k0, m.k1, b0);
             float vx, vy, vz;
@@ -400,7 +402,11 @@ __global__ void __launch_bounds__(PIC1D_NT, STAGE ? 3 : 4) k_mcc(MccArgs a) {
         }
         __syncthreads();
     }
-    mcc_flush_counts(m, cnt);
+    mcc_flush_counts(m, cnt);  // events and over-cap; its null count is (0 candidates - events) ...
+    if (tid == 0 && n_cand_block) {  // ... and the candidates complete both (unsigned wrap-around is exact)
+        atomicAdd(&sp.n_candidates, n_cand_block);
+        atomicAdd(&sp.n_events[0], n_cand_block);
+    }
 }
 
 // ---- the ionisation pairs (L203), in ascending parent-slot order ---------------------------------------
