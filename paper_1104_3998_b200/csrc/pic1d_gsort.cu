@@ -18,6 +18,7 @@ namespace {
 
 #define GS_NT 256
 #define GS_PT 32  // particles per thread and cell at most: n_max <= GS_NT * GS_PT = 8192
+#define GS_U 8    // of them in flight together
 
 struct GsState {
     ull absorbed_left, absorbed_right, moved_near, moved_far;
@@ -46,22 +47,36 @@ __global__ void __launch_bounds__(GS_NT) k_gs_push(GsArgs a) {
         if (tid == 0) { s_top = a.n_max; s_holes = 0; s_nh = 0; s_nd = 0; s_abs[0] = 0; s_abs[1] = 0; }
         __syncthreads();
         unsigned rej = 0;  // bit it: my particle tid + it * GS_NT left the cell
-        for (int it = 0; it < GS_PT; ++it) {
-            const int j = tid + it * GS_NT;
-            if (j >= N) break;
-            float x = a.x[base + j], vx = a.vx[base + j];
-            int dummy = 0;
-            const int key = push_particle<0>(x, vx, true, a.E32, a.kappa, a.n_cells, a.fNc, a.inv_r, 0, norefl, 0u, 0u, dummy);
-            if (key == c) {
-                a.x[base + j] = x; a.vx[base + j] = vx;
-                continue;
+        // GS_U particles per thread at a time: their loads are independent and in flight together (a thread's own
+        // slots j < N are read before anything is written to them; rejected particles go to slots >= N)
+        for (int it0 = 0; it0 < GS_PT && it0 * GS_NT < N; it0 += GS_U) {
+            float xs[GS_U], vs[GS_U];
+#pragma unroll
+            for (int u = 0; u < GS_U; ++u) {
+                const int j = tid + (it0 + u) * GS_NT;
+                xs[u] = 0.0f; vs[u] = 0.0f;
+                if (j < N) { xs[u] = __ldcs(a.x + base + j); vs[u] = __ldcs(a.vx + base + j); }
             }
-            rej |= 1u << it;
-            atomicAdd(&s_holes, 1);
-            if (key < 0) { atomicAdd(&s_abs[key == -1 ? 0 : 1], 1); continue; }  // left the box (L41): dropped
-            const int idx = atomicSub(&s_top, 1) - 1;  // step 1a: N_index counts down from the end of the cell
+#pragma unroll
+            for (int u = 0; u < GS_U; ++u) {
+                const int it = it0 + u, j = tid + it * GS_NT;
+                if (j >= N) continue;
+                float x = xs[u], vx = vs[u];
+                int dummy = 0;
+                const int key = push_particle<0>(x, vx, true, a.E32, a.kappa, a.n_cells, a.fNc, a.inv_r, 0, norefl, 0u, 0u, dummy);
+                a.x[base + j] = x; a.vx[base + j] = vx;  // in place, whether it stays or not
+                if (key != c) rej |= 1u << it;           // the rare path is taken after the loop
+            }
+        }
+        // step 1a for the thread's rejected particles (few): to the end of the cell through the shared counter
+        if (rej) atomicAdd(&s_holes, __popc(rej));
+        for (unsigned todo = rej; todo; todo &= todo - 1u) {
+            const int j = tid + (__ffs(todo) - 1) * GS_NT;
+            const float x = a.x[base + j];  // this thread's own store above
+            if (!(x >= 0.0f && x < a.fNc)) { atomicAdd(&s_abs[x < 0.0f ? 0 : 1], 1); continue; }  // left the box (L41): dropped
+            const int idx = atomicSub(&s_top, 1) - 1;  // N_index counts down from the end of the cell
             if (idx < N) { atomicOr(&a.st->err, 1u); continue; }  // no free slot left: dropped, sticky error
-            a.x[base + idx] = x; a.vx[base + idx] = vx;
+            a.x[base + idx] = x; a.vx[base + idx] = a.vx[base + j];
             a.vy[base + idx] = a.vy[base + j]; a.vz[base + idx] = a.vz[base + j];
         }
         __syncthreads();
