@@ -363,10 +363,12 @@ def test_cold_plasma_frequency_on_gpu():
     g.close()
 
 
-@pytest.mark.parametrize("cfg_id,steps", [(1, 3), (2, 3), (3, 2)])
-def test_full_size_configs_single_steps(cfg_id, steps):
-    """BASELINE.json configs 1-3 at their full sizes (config 3 at sort ratio 1), every output compared"""
-    o, g, p = _mk(W.make_params(cfg_id))
+@pytest.mark.parametrize("cfg_id,steps,ratio", [(1, 3, 1.0), (2, 3, 1.0), (3, 2, 1.0),
+                                                (3, 1, 0.5), (3, 1, 2.0), (3, 1, 16.0)])   # config 3's sweep at full size
+def test_full_size_configs_single_steps(cfg_id, steps, ratio):
+    """BASELINE.json configs 1-3 at their full sizes, config 3 at every ratio of its sweep (r = 4 runs in the long-run
+    test), every output compared"""
+    o, g, p = _mk(W.make_params(cfg_id, sort_ratio=ratio))
     from oracle import oracle as O
     run_compared_steps(o, g, p, steps)
     o.close(); g.close()
