@@ -10,7 +10,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpic1d.so")
-SOURCES = ["pic1d.cu", "pic1d_gsort.cu"]
+SOURCES = ["pic1d.cu", "pic1d_gsort.cu", "pic1d_field_static.cu"]
 DEPS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh")))   # every source under csrc/
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false",
               "-std=c++17", "-shared", "-Xcompiler", "-fPIC"]
@@ -20,7 +20,7 @@ def needs_build():
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, d) for d in DEPS] + [os.path.join(HERE, "..", "include", h) for h in ("pic1d.h", "pic1d_gsort.h")]
+    deps = [os.path.join(CSRC, d) for d in DEPS] + [os.path.join(HERE, "..", "include", h) for h in ("pic1d.h", "pic1d_gsort.h", "pic1d_static.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

@@ -7,6 +7,7 @@ import re
 from paper_1104_3998_b200 import build as B
 from paper_1104_3998_b200 import pic1d as G
 from paper_1104_3998_b200 import gsort as GS
+from paper_1104_3998_b200 import field_static as FS
 from paper_1104_3998_b200 import workloads as W
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -14,7 +15,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def _declared():
     names = set()
-    for h in ("pic1d.h", "pic1d_gsort.h"):
+    for h in ("pic1d.h", "pic1d_gsort.h", "pic1d_static.h"):
         src = open(os.path.join(ROOT, "include", h)).read()
         src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
         names |= set(re.findall(r"\b(pic1d_[a-z0-9_E]+)\s*\(", src))
@@ -25,7 +26,7 @@ def test_library_exports_every_declared_symbol():
     B.build()
     lib = G.load_library()
     names = _declared()
-    assert len(names) >= 22 and set(G.EXPORTS) | set(GS.EXPORTS) == set(names)
+    assert len(names) >= 22 and set(G.EXPORTS) | set(GS.EXPORTS) | set(FS.EXPORTS) == set(names)
     for n in names:
         assert getattr(lib, n) is not None
 
