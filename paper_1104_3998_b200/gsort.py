@@ -4,7 +4,7 @@ import ctypes as C
 
 import numpy as np
 
-from .pic1d import load_library, Pic1DError, _ptr
+from .pic1d import load_library, Pic1DError, _ptr, _adopt
 
 EXPORTS = ["pic1d_gsort_workspace_bytes", "pic1d_gsort_create", "pic1d_gsort_load", "pic1d_gsort_set_E32",
            "pic1d_gsort_step", "pic1d_gsort_get", "pic1d_gsort_n_sort_cells", "pic1d_gsort_destroy"]
@@ -24,6 +24,8 @@ class GappedSort:
             raise Pic1DError("pic1d_gsort_workspace_bytes", rc)
         self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
         self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
+        self._torch = torch
+        _adopt(torch, self.stream, self.device, [self.workspace])
         self.h = C.c_void_p()
         rc = self.lib.pic1d_gsort_create(C.c_int(n_cells), C.c_double(sort_inv_ratio), C.c_int(n_max), C.c_double(kappa),
                                          C.c_void_p(self.workspace.data_ptr()), nbytes, C.c_void_p(self.stream.cuda_stream),
@@ -35,6 +37,7 @@ class GappedSort:
 
     def close(self):
         if getattr(self, "h", None):
+            self.stream.synchronize()       # the workspace goes back to torch's allocator
             self.lib.pic1d_gsort_destroy(self.h)
             self.h = C.c_void_p()
             self.workspace = None
@@ -50,13 +53,20 @@ class GappedSort:
         on_device = 1 if all(hasattr(a, "is_cuda") and a.is_cuda for a in arrs) else 0
         if not on_device:
             arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in arrs]
+        else:   # produced on torch's current stream, copied on ours
+            arrs = [a.contiguous() for a in arrs]
+            assert all(a.dtype == self._torch.float32 for a in arrs)
+            _adopt(self._torch, self.stream, self.device, arrs)
         rc = self.lib.pic1d_gsort_load(self.h, C.c_int64(int(arrs[0].shape[0])), *[_ptr(a) for a in arrs], C.c_int(on_device))
         if rc:
             raise Pic1DError("pic1d_gsort_load", rc)
 
     def set_E32(self, e32):
         on_device = 1 if hasattr(e32, "is_cuda") and e32.is_cuda else 0
-        a = e32 if on_device else np.ascontiguousarray(e32, dtype=np.float32)
+        a = e32.contiguous() if on_device else np.ascontiguousarray(e32, dtype=np.float32)
+        if on_device:
+            assert a.dtype == self._torch.float32
+            _adopt(self._torch, self.stream, self.device, [a])
         rc = self.lib.pic1d_gsort_set_E32(self.h, _ptr(a), C.c_int(int(a.shape[0])), C.c_int(on_device))
         if rc:
             raise Pic1DError("pic1d_gsort_set_E32", rc)

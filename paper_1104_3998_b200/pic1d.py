@@ -29,7 +29,7 @@ _DBG_DTYPE = {DBG_X: np.float32, DBG_VX: np.float32, DBG_VY: np.float32, DBG_VZ:
 EXPORTS = ["pic1d_workspace_bytes", "pic1d_create", "pic1d_load_particles", "pic1d_step",
            "pic1d_get_rho_phi_E", "pic1d_moments", "pic1d_destroy", "pic1d_n_nodes",
            "pic1d_n_sort_cells", "pic1d_step_index", "pic1d_last_cuda_error", "pic1d_launch_count",
-           "pic1d_step_timed", "pic1d_debug_count", "pic1d_debug_get", "pic1d_debug_set_E32",
+           "pic1d_graph_launch_count", "pic1d_step_timed", "pic1d_debug_count", "pic1d_debug_get", "pic1d_debug_set_E32",
            "pic1d_debug_set_state"]
 
 
@@ -80,6 +80,7 @@ def load_library():
         lib = C.CDLL(LIB_PATH)
         lib.pic1d_last_cuda_error.restype = C.c_char_p
         lib.pic1d_launch_count.restype = C.c_int64
+        lib.pic1d_graph_launch_count.restype = C.c_int64
         lib.pic1d_step_index.restype = C.c_uint32
         _lib = lib
     return _lib
@@ -117,6 +118,20 @@ def _ptr(a):
     return C.c_void_p(a.data_ptr())
 
 
+def _adopt(torch, stream, device, tensors):
+    """Order `stream` after torch's current stream and tell the caching allocator that `stream` uses `tensors`.
+
+    The handle runs on a stream of its own, but CUDA tensors handed to it (and its workspace) are produced or
+    allocated on torch's current stream.  Without the wait a device-to-device copy could read a tensor before
+    the kernel that fills it has run; without record_stream a temporary (.contiguous()) or the workspace could be
+    handed out again by the allocator while our stream still reads or writes it."""
+    cur = torch.cuda.current_stream(device)
+    if cur != stream:
+        stream.wait_stream(cur)
+        for t in tensors:
+            t.record_stream(stream)
+
+
 class Pic1D:
     """One simulation handle on the current CUDA device; methods mirror the C calls."""
 
@@ -137,6 +152,7 @@ class Pic1D:
         self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
         # a stream of its own: the legacy default stream cannot be captured into a CUDA graph
         self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
+        _adopt(torch, self.stream, self.device, [self.workspace])
         self.h = C.c_void_p()
         rc = self.lib.pic1d_create(C.byref(self.cfg), C.c_void_p(self.workspace.data_ptr()), nbytes,
                                    C.c_void_p(self.stream.cuda_stream), C.byref(self.h))
@@ -147,6 +163,7 @@ class Pic1D:
 
     def close(self):
         if getattr(self, "h", None):
+            self.stream.synchronize()       # the workspace goes back to torch's allocator: nothing may still use it
             self.lib.pic1d_destroy(self.h)
             self.h = C.c_void_p()
             self.workspace = None
@@ -169,6 +186,8 @@ class Pic1D:
             on_device = 1 if arrs[0].is_cuda else 0
             arrs = [a.contiguous() for a in arrs]
             assert all(a.dtype == self._torch.float32 for a in arrs)
+            if on_device:   # produced on torch's current stream, copied on ours
+                _adopt(self._torch, self.stream, self.device, arrs)
         else:
             arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in arrs]
         n = int(arrs[0].shape[0])
@@ -248,6 +267,11 @@ class Pic1D:
     @property
     def launch_count(self):
         return int(self.lib.pic1d_launch_count(self.h))
+
+    @property
+    def graph_launch_count(self):
+        """CUDA-graph replays (two steps each) so far; -1 = capture failed once, plain launches since"""
+        return int(self.lib.pic1d_graph_launch_count(self.h))
 
     def synchronize(self):
         self.stream.synchronize()
