@@ -307,7 +307,7 @@ def main():
     m0 = live()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    l0 = sim.launch_count
+    l0, gl0 = sim.launch_count, sim.graph_launch_count
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(sim.stream)
@@ -317,6 +317,7 @@ def main():
     clocks = sampler.result()
     ms = e0.elapsed_time(e1)
     launches = sim.launch_count - l0
+    graph_replays = sim.graph_launch_count - gl0 if sim.graph_launch_count >= 0 else 0   # checked, not assumed
     m1 = live()
     n_mean = 0.5 * (sum(m["count"] for m in m0) + sum(m["count"] for m in m1))
     ms_max, n_total = R.reduce_replicas(ms, n_mean, dev)
@@ -464,7 +465,7 @@ def main():
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "capture_masks": False,
                        "mcc": {("electrons", "ions")[q]: ("folded into the scatter" if folded[q] else "own pass (k_mcc)") for q in range(ns)},
-                       "cuda_graph": not args.no_graph, "mcc_beside_field_solve": not args.no_overlap,
+                       "cuda_graph": graph_replays > 0, "graph_replays_in_timed_region": graph_replays, "mcc_beside_field_solve": not args.no_overlap,
                        "sort": ("electrons and ions: warp tiles of 256 slots" if p["flags"] & 4 else
                                 "electrons: block tiles of 2048 slots (staged scatter); ions: warp tiles of 256 slots")},
             "clocks": clocks, "gpu_launches": launches,

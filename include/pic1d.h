@@ -180,6 +180,10 @@ uint32_t pic1d_step_index(const pic1d_t* h);
 const char* pic1d_last_cuda_error(const pic1d_t* h);
 /* number of kernel launches enqueued by this handle since creation */
 int64_t pic1d_launch_count(const pic1d_t* h);
+/* number of CUDA-graph replays (two steps each) pic1d_step has launched since creation; -1 once a capture or an
+ * instantiation has failed (e.g. on the legacy default stream): the handle then launches every kernel itself for
+ * good, with identical results.  0 with PIC1D_FLAG_NO_GRAPH. */
+int64_t pic1d_graph_launch_count(const pic1d_t* h);
 
 /* Per-kernel timing (host API, synchronises): runs ONE step with CUDA events between the kernels
  * and writes up to max_kernels entries of (name, milliseconds).  Returns the number of entries. */

@@ -76,7 +76,9 @@ struct pic1d {
     cudaStream_t side;              // collisions run here beside the deposit and the field solve
     cudaEvent_t ev_fork, ev_join;
     bool null_ready;                // the null-test masks of the NEXT step have been enqueued (by the previous step)
-    cudaGraphExec_t graph[2];       // two captured steps, per parity of the sort buffers at their start
+    cudaGraphExec_t graph[4];       // two captured steps, per parity of BOTH species' sort buffers at their start
+    bool graph_off;                 // a capture or an instantiation failed once: plain launches from then on
+    int64_t graph_launches;         // replays so far
     int64_t launches_per_2steps;
     bool timing;
     std::vector<TimeMark> marks;
@@ -120,7 +122,9 @@ int validate_cfg(const pic1d_config_t* c) {
     for (int s = 0; s < c->n_species; ++s) {
         int64_t cap = c->sp[s].capacity;
         if (cap < 4096 || cap % 4096 != 0 || cap > (1ll << 30)) return PIC1D_ERR_ARG;
+        if (!(c->coul_A[s] >= 0.0) || !std::isfinite(c->coul_A[s])) return PIC1D_ERR_ARG;  // 0 = off
     }
+    if (!(c->e_reflect >= 0.0 && c->e_reflect <= 1.0)) return PIC1D_ERR_ARG;  // a probability (also rejects NaN)
     return PIC1D_OK;
 }
 
@@ -532,6 +536,16 @@ __global__ void k_set_count(DevState* st, int s, int n) {
 }
 __global__ void k_clear_err(DevState* st) { st->err = 0; st->step = 0; st->step_next = 0; st->n_abs = 0; }
 
+// The one exit of a handle: every CUDA object it owns (pic1d{} starts them all as null), then the handle.
+void free_handle(pic1d* h) {
+    for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
+    for (cudaGraphExec_t g : h->graph) if (g) cudaGraphExecDestroy(g);
+    if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); }
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->ev_join) cudaEventDestroy(h->ev_join);
+    delete h;
+}
+
 }  // namespace
 
 // =================================== C-ABI ===========================================================
@@ -566,11 +580,10 @@ int pic1d_create(const pic1d_config_t* cfg, void* workspace, size_t workspace_by
         return PIC1D_ERR_CUDA;
     }
     h->num_sms = prop.multiProcessorCount;
-    h->side = nullptr; h->graph[0] = h->graph[1] = nullptr;
     if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess) {
-        delete h;
+        free_handle(h);
         return PIC1D_ERR_CUDA;
     }
     setup_launch(h);
@@ -582,7 +595,7 @@ int pic1d_create(const pic1d_config_t* cfg, void* workspace, size_t workspace_by
         ok = ok && ck(h, cudaMemsetAsync(h->ion_nb, 0, sizeof(int) * h->sp[0].n_mcc_tiles, h->stream));
     }
     ok = ok && ck(h, cudaMemsetAsync(h->E32, 0, sizeof(float) * (h->nodes + 1), h->stream));
-    if (!ok || !ck(h, cudaGetLastError())) { delete h; return PIC1D_ERR_CUDA; }
+    if (!ok || !ck(h, cudaGetLastError())) { free_handle(h); return PIC1D_ERR_CUDA; }
     *out = h;
     return PIC1D_OK;
 }
@@ -590,10 +603,7 @@ int pic1d_create(const pic1d_config_t* cfg, void* workspace, size_t workspace_by
 int pic1d_destroy(pic1d_t* h) {
     if (!h) return PIC1D_OK;
     cudaStreamSynchronize(h->stream);
-    for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
-    for (int g = 0; g < 2; ++g) if (h->graph[g]) cudaGraphExecDestroy(h->graph[g]);
-    if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); cudaEventDestroy(h->ev_fork); cudaEventDestroy(h->ev_join); }
-    delete h;
+    free_handle(h);
     return PIC1D_OK;
 }
 
@@ -667,12 +677,17 @@ int pic1d_step(pic1d_t* h, int n_steps) {
     // once per buffer parity into a CUDA graph and replayed: every per-step quantity (step index, particle
     // counts, tickets) lives in DevState on the device, no kernel argument changes from step to step.
     if (!h->null_ready && n_steps > 0) { enqueue_step(h); k = 1; }  // (a captured step counts on the masks computed ahead)
-    if (!(h->cfg.flags & PIC1D_FLAG_NO_GRAPH)) {
+    if (!(h->cfg.flags & PIC1D_FLAG_NO_GRAPH) && !h->graph_off) {
         while (n_steps - k >= 2) {
-            const int par = h->sp[0].cur;
+            // the baked kernel arguments depend on which buffer of EVERY species is current
+            const int par = h->sp[0].cur | (h->cfg.n_species > 1 ? h->sp[1].cur << 1 : 0);
             if (!h->graph[par]) {
                 cudaGraph_t g = nullptr;
-                if (cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); break; }
+                if (cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+                    cudaGetLastError();
+                    h->graph_off = true;  // e.g. the legacy default stream: do not try again every call
+                    break;
+                }
                 const int64_t l0 = h->launches;
                 const uint32_t s0 = h->step;
                 enqueue_step(h);
@@ -684,11 +699,13 @@ int pic1d_step(pic1d_t* h, int n_steps) {
                     if (g) cudaGraphDestroy(g);
                     h->graph[par] = nullptr;
                     cudaGetLastError();
+                    h->graph_off = true;
                     break;
                 }
                 cudaGraphDestroy(g);
             }
             if (!ck(h, cudaGraphLaunch(h->graph[par], h->stream))) return PIC1D_ERR_CUDA;
+            ++h->graph_launches;
             h->launches += h->launches_per_2steps;
             h->step += 2u;
             k += 2;
@@ -775,6 +792,7 @@ int pic1d_n_sort_cells(const pic1d_t* h) { return h ? h->n_sc : PIC1D_ERR_ARG; }
 uint32_t pic1d_step_index(const pic1d_t* h) { return h ? h->step : 0u; }
 const char* pic1d_last_cuda_error(const pic1d_t* h) { return h ? cudaGetErrorString(h->last_err) : "null handle"; }
 int64_t pic1d_launch_count(const pic1d_t* h) { return h ? h->launches : 0; }
+int64_t pic1d_graph_launch_count(const pic1d_t* h) { return !h ? 0 : h->graph_off ? -1 : h->graph_launches; }
 
 int pic1d_debug_count(pic1d_t* h, int what, int s, int64_t* count_out) {
     if (!h || !count_out || s < 0 || s >= h->cfg.n_species || !h->ready) return PIC1D_ERR_ARG;

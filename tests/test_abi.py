@@ -50,6 +50,21 @@ def test_struct_sizes_and_workspace_query():
     c = G.make_config(W.make_params(0))
     c.sp[0].capacity = 5000     # not a multiple of 4096
     assert lib.pic1d_workspace_bytes(C.byref(c), C.byref(n)) == G.ERR_ARG
+    for field, bad in (("e_reflect", -0.1), ("e_reflect", 1.5), ("e_reflect", float("nan"))):
+        c = G.make_config(W.make_params(0))
+        setattr(c, field, bad)   # a probability
+        assert lib.pic1d_workspace_bytes(C.byref(c), C.byref(n)) == G.ERR_ARG, (field, bad)
+    for s in (0, 1):
+        for bad in (-1.0, float("inf"), float("nan")):
+            c = G.make_config(W.make_params(0))
+            c.coul_A[s] = bad
+            assert lib.pic1d_workspace_bytes(C.byref(c), C.byref(n)) == G.ERR_ARG, (s, bad)
+    c = G.make_config(W.make_params(0))
+    c.e_reflect, c.coul_A[0], c.coul_A[1] = 1.0, 0.0, 2.5
+    assert lib.pic1d_workspace_bytes(C.byref(c), C.byref(n)) == 0
+    h = C.c_void_p()            # pic1d_create validates the same way, before touching the device
+    c.e_reflect = 2.0
+    assert lib.pic1d_create(C.byref(c), C.c_void_p(256), C.c_size_t(1 << 30), None, C.byref(h)) == G.ERR_ARG
 
 
 def test_product_path_does_not_import_oracle():
