@@ -461,12 +461,30 @@ static void mcc(orc_t* o) {
  * <delta^2> = coul_A n / u^3 (coul_A = q^4 w lnLambda dt / (8 pi eps0^2 m_r^2 V_cell), m_r = m/2,
  * in normalised units, computed by the caller), azimuth phi uniform; u is rotated, each partner takes
  * half of the change: momentum and energy of the pair are conserved.
- * Pairing (R23; the paper gives none, Takizuka-Abe pair at random): a random affine
- * permutation pi(k) = (a k + b) mod n of the cell's sorted slots, a coprime to n, from
- * philox(cell, step, COUL + s, 0); pairs are (pi(2m), pi(2m+1)); for odd n slot pi(n-1) sits out. */
-static uint32_t gcd_u32(uint32_t a, uint32_t b) {
-    while (b) { uint32_t t = a % b; a = b; b = t; }
-    return a;
+ * Pairing (R23; the paper gives none, Takizuka-Abe pair at random): a keyed pseudo-random
+ * permutation pi of the cell's sorted slots 0 .. n-1; pairs are (pi(2m), pi(2m+1)); for odd n slot pi(n-1)
+ * sits out (Takizuka-Abe's three-particle rule for odd n is NOT used).  pi is a 4-round balanced Feistel
+ * network on 2h bits, h the smallest integer with 4^h >= n, keyed by the four words of
+ * philox(cell, step, COUL + s, 0), made a permutation of [0, n) by cycle walking (apply again while the value
+ * is >= n: a cycle of a permutation of [0, 4^h) that starts below n comes back below n).  Any pairing of the
+ * cell can come out, unlike the single-stride pairs of an affine map (a m + b) mod n. */
+static uint32_t coul_mix(uint32_t z) { /* round function: an integer hash, the low h bits are used */
+    z *= 0x9E3779B1u; z ^= z >> 15; z *= 0x85EBCA77u; z ^= z >> 13;
+    return z;
+}
+
+static uint32_t coul_perm(uint32_t m, uint32_t n, uint32_t h, const uint32_t w[4]) {
+    const uint32_t mask = (1u << h) - 1u;
+    uint32_t x = m;
+    do {
+        uint32_t L = x >> h, R = x & mask;
+        for (int r = 0; r < 4; ++r) {
+            uint32_t t = L ^ (coul_mix(R ^ w[r]) & mask);
+            L = R; R = t;
+        }
+        x = (L << h) | R;
+    } while (x >= n);
+    return x;
 }
 
 static void coulomb(orc_t* o) {
@@ -482,13 +500,12 @@ static void coulomb(orc_t* o) {
             uint32_t w[4];
             philox4x32_10((uint32_t)k, o->step, STREAM_COUL + (uint32_t)s, 0u, (uint32_t)c->seed,
                           (uint32_t)(c->seed >> 32), w);
-            uint32_t a = n > 2 ? 1u + w[0] % (n - 1u) : 1u; /* in [1, n) */
-            while (gcd_u32(a, n) != 1u) a = a + 1u == n ? 1u : a + 1u;
-            uint32_t b = w[1] % n;
+            uint32_t h = 1;
+            while ((1ull << (2 * h)) < n) ++h; /* 4^h >= n */
             float fn = (float)n;
             for (uint32_t m = 0; m + 1 < n; m += 2) {
-                uint32_t ia = off + (uint32_t)(((uint64_t)a * m + b) % n);
-                uint32_t ib = off + (uint32_t)(((uint64_t)a * (m + 1) + b) % n);
+                uint32_t ia = off + coul_perm(m, n, h, w);
+                uint32_t ib = off + coul_perm(m + 1, n, h, w);
                 p->partner[ia] = (int32_t)ib; p->partner[ib] = (int32_t)ia;
                 p->m.n_pairs++;
                 float u4[4];

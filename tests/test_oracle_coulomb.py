@@ -48,6 +48,52 @@ def test_pairing_is_a_perfect_matching_inside_each_cell(n_cells, ratio, n):
     assert np.mean(seen[0] == seen[1]) < 0.2 and np.mean(seen[1] == seen[2]) < 0.2   # new partners every step
 
 
+def _partners_of_one_cell(n, steps, seed=5):
+    """partner arrays (slot numbers inside the cell) of a single sort cell of n particles over `steps` steps"""
+    rng = np.random.default_rng(seed)
+    p = _box(n, 1e-9, n_cells=8, sort_ratio=8.0, seed=seed)
+    o = O.Oracle(p)
+    x = (rng.random(n, dtype=np.float32) * 8).astype(np.float32)
+    v = (rng.normal(size=(3, n)) * 1e-4).astype(np.float32)
+    load(o, [(x, v[0], v[1], v[2])])
+    out = []
+    for _ in range(steps):
+        o.step(1)
+        out.append(o.debug_get(O.PARTNER).copy())
+    return out
+
+
+def test_every_pairing_of_four_particles_comes_out_equally_often():
+    """n = 4 has three perfect matchings, 01|23, 02|13, 03|12; random pairing (Takizuka-Abe) draws each with
+    probability 1/3.  (An affine map (a m + b) mod 4 can never pair slots 0 and 2: this pin rejects it.)"""
+    steps = 600
+    count = {1: 0, 2: 0, 3: 0}
+    for part in _partners_of_one_cell(4, steps):
+        assert sorted(part[part]) == [0, 1, 2, 3]
+        count[int(part[0])] += 1
+    for k in (1, 2, 3):
+        assert abs(count[k] - steps / 3) <= 4.5 * np.sqrt(steps * (1 / 3) * (2 / 3)), count
+
+
+def test_pair_distances_in_a_cell_are_not_a_single_stride():
+    """the slot distance |i - partner(i)| of random pairs of n slots has the triangular law P(d) = 2 (n - d) /
+    (n (n - 1)); pairs built from one stride would all share one or two distances"""
+    n, steps = 101, 40
+    d = np.concatenate([np.abs(np.arange(n) - part)[part >= 0] for part in _partners_of_one_cell(n, steps)])
+    assert d.shape[0] == steps * (n - 1)
+    for part in _partners_of_one_cell(n, 3):
+        assert np.unique(np.abs(np.arange(n) - part)[part >= 0]).shape[0] > 25
+    hist = np.bincount(d, minlength=n)[1:] / 2                      # pairs per distance (each pair counted twice)
+    want = steps * (n // 2) * 2 * (n - np.arange(1, n)) / (n * (n - 1))
+    # chi-square over 10 bands of distances (each band has dozens of expected pairs)
+    bands = np.array_split(np.arange(n - 1), 10)
+    chi2 = sum((hist[b].sum() - want[b].sum()) ** 2 / want[b].sum() for b in bands)
+    assert chi2 < 35.0, chi2                                        # 9 degrees of freedom: P(chi2 > 35) < 1e-4
+    # who sits out of an odd cell is uniform too: not always the same slot
+    out = [int(np.nonzero(part < 0)[0][0]) for part in _partners_of_one_cell(n, steps)]
+    assert len(set(out)) > steps // 2
+
+
 def test_every_pair_conserves_momentum_and_energy():
     n = 20000
     rng = np.random.default_rng(2)
