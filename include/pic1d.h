@@ -105,7 +105,10 @@ typedef struct pic1d_config {
                               featured, electrons are inserted at the boundaries"); 0 = off */
     double coul_A[PIC1D_MAX_SPECIES]; /* binary Coulomb collisions between the like particles of a sort cell (L69, L75,
                               L221, L259; Takizuka-Abe): <tan^2(theta/2)> = coul_A n_cell / u^3 with u in cells/step,
-                              coul_A = q^4 w lnLambda dt / (8 pi eps0^2 m_r^2 A_e r dx) (dt/dx)^3, m_r = m/2; 0 = off */
+                              coul_A = q^4 w lnLambda dt / (8 pi eps0^2 m_r^2 A_e r dx) (dt/dx)^3, m_r = m/2; 0 = off.
+                              Pairing: a keyed pseudo-random permutation of the cell's sorted slots, new every step,
+                              consecutive images are partners; in a cell with an odd count one particle sits the step
+                              out (Takizuka-Abe instead collide the first three among themselves) */
 } pic1d_config_t;
 
 typedef struct pic1d_moments {

@@ -7,8 +7,10 @@
 // (1977) 205) needs: the n particles of a sort cell are paired, a pair with relative velocity u is scattered by
 // theta with tan(theta/2) = delta ~ N(0, coul_A n / u^3) and a uniform azimuth, each partner takes half of the
 // change of u (like particles: equal mass and weight), so momentum and energy of every pair are conserved.
-// Pairing (R23): a random affine permutation pi(m) = (a m + b) mod n of the cell's sorted slots, a
-// coprime to n, from philox(cell, step, COUL + s, 0); pairs (pi(2m), pi(2m+1)); for odd n slot pi(n-1) sits out.
+// Pairing (R23): a keyed pseudo-random permutation pi of the cell's sorted slots -- four balanced Feistel
+// rounds on 2h bits (4^h >= n) keyed by philox(cell, step, COUL + s, 0), cycle-walked into [0, n) -- so that any
+// pairing of the cell can come out; pairs (pi(2m), pi(2m+1)); for odd n slot pi(n-1) sits out (not Takizuka-Abe's
+// three-particle rule).  Every thread evaluates pi for its own pairs: integer work, bit-identical to the oracle's.
 // One block per sort cell, one thread per pair; the cell's velocities (12 B x n) are gathered through L1.
 // fp32 operations in the order the oracle states them (-fmad=false: nothing is contracted).
 #pragma once
@@ -25,9 +27,21 @@ struct CoulombArgs {
     uint32_t k0, k1;
 };
 
-__device__ __forceinline__ unsigned gcd_u32(unsigned a, unsigned b) {
-    while (b) { const unsigned t = a % b; a = b; b = t; }
-    return a;
+__device__ __forceinline__ unsigned coul_feistel(unsigned m, unsigned n, unsigned h, const uint32_t (&w)[4]) {
+    const unsigned mask = (1u << h) - 1u;
+    unsigned x = m;
+    do {  // cycle walking: a cycle of the permutation of [0, 4^h) that starts below n returns below n
+        unsigned L = x >> h, R = x & mask;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            unsigned z = (R ^ w[r]) * 0x9E3779B1u;
+            z ^= z >> 15; z *= 0x85EBCA77u; z ^= z >> 13;
+            const unsigned t = L ^ (z & mask);
+            L = R; R = t;
+        }
+        x = (L << h) | R;
+    } while (x >= n);
+    return x;
 }
 
 __global__ void __launch_bounds__(PIC1D_NT) k_coulomb(CoulombArgs a) {
@@ -43,14 +57,13 @@ __global__ void __launch_bounds__(PIC1D_NT) k_coulomb(CoulombArgs a) {
         }
         uint32_t w[4];
         philox4x32_10((uint32_t)k, step, stream, 0u, a.k0, a.k1, w);  // every thread: the cell's permutation
-        unsigned am = n > 2u ? 1u + w[0] % (n - 1u) : 1u;             // in [1, n)
-        while (gcd_u32(am, n) != 1u) am = am + 1u == n ? 1u : am + 1u;
-        const unsigned bm = w[1] % n;
+        unsigned h = 1u;
+        while ((1ull << (2u * h)) < n) ++h;  // 4^h >= n
         const float fn = (float)n;
-        if (a.partner && (n & 1u) && tid == 0) a.partner[off + (unsigned)(((ull)am * (n - 1u) + bm) % n)] = -1;
+        if (a.partner && (n & 1u) && tid == 0) a.partner[off + coul_feistel(n - 1u, n, h, w)] = -1;
         for (unsigned m = 2u * tid; m + 1u < n; m += 2u * PIC1D_NT) {
-            const unsigned ia = off + (unsigned)(((ull)am * m + bm) % n);
-            const unsigned ib = off + (unsigned)(((ull)am * (m + 1u) + bm) % n);
+            const unsigned ia = off + coul_feistel(m, n, h, w);
+            const unsigned ib = off + coul_feistel(m + 1u, n, h, w);
             if (a.partner) { a.partner[ia] = (int)ib; a.partner[ib] = (int)ia; }
             ++n_pairs;
             const float vxa = a.vx[ia], vya = a.vy[ia], vza = a.vz[ia];
