@@ -124,3 +124,38 @@ def test_ionisation_pair_keeps_rho_neutral():
     me, mi = o.moments(0), o.moments(1)
     assert mi["count"] > 0
     assert me["density"].sum() - mi["density"].sum() == 50000 - (me["absorbed_left"] + me["absorbed_right"])
+
+
+def test_ionisation_capacity_drop_keeps_the_first_births():
+    """The capacity-drop branch of the ionisation births (L203; R14): a pair is born only while BOTH
+    arrays have a free slot; the births that fit are the ones of the lowest parent slots, the rest are counted as
+    dropped (once per species) and the sticky capacity error is raised; the parent's own collision happens either
+    way.  Pinned against the SAME step with room for everybody."""
+    n = 12288 - 20                           # ~50 ionisations per step at this pressure: 20 slots do not hold them
+    res = {}
+    for name, cap_e in (("room", 16384), ("full", 12288)):
+        o, p, g = _beam(60.0, n=n)           # well above the ionisation threshold
+        o.close()
+        p["species"][0]["capacity"] = cap_e
+        p["species"][1]["capacity"] = 4096 * 4
+        o = O.Oracle(p)
+        x = (np.arange(n, dtype=np.float32) % 8 + 0.5).astype(np.float32)
+        z = np.zeros(n, np.float32)
+        empty = (np.zeros(0, np.float32),) * 4
+        load(o, [(x, z, np.full(n, g, np.float32), z), empty])
+        rc = o.step(1)
+        me, mi = o.moments(0), o.moments(1)
+        arr = [o.debug_get(w, 0) for w in (O.X, O.VX, O.VY, O.VZ)]
+        ions = [o.debug_get(w, 1) for w in (O.X, O.VX, O.VY, O.VZ)]
+        res[name] = (rc, me, mi, arr, ions, o.debug_get(O.MASK, 0))
+    (rc_r, me_r, mi_r, a_r, i_r, k_r), (rc_f, me_f, mi_f, a_f, i_f, k_f) = res["room"], res["full"]
+    free = 12288 - n
+    assert rc_r == 0 and me_r["dropped"] == 0 and me_r["births"] == me_r["n_events"][3] > 2 * free
+    assert rc_f == -2 and me_f["births"] == free and mi_f["births"] == free
+    assert me_f["dropped"] == me_r["births"] - free and mi_f["dropped"] == me_f["dropped"]
+    assert np.array_equal(k_r, k_f) and me_f["n_events"] == me_r["n_events"]     # every parent still collides
+    assert me_f["count"] == n + free and mi_f["count"] == free
+    for a, b in zip(a_r, a_f):          # parents (all n slots) and the first `free` new electrons: identical
+        assert np.array_equal(a[:n + free], b)
+    for a, b in zip(i_r, i_f):
+        assert np.array_equal(a[:free], b)

@@ -177,6 +177,44 @@ def test_secondary_emission_binomial_and_placement():
     assert abs(np.mean(vy)) < 4 * p["see_vth"] / np.sqrt(k)
 
 
+def test_secondary_emission_capacity_drop_keeps_the_first_emitters():
+    """The capacity-drop branch of the injection (L41; R10/R19): when the electron arrays fill up,
+    the emitters that still fit -- in the order of the absorbed-ion list -- are injected, the rest are counted
+    as dropped and the sticky capacity error is raised.  Pinned against the SAME step with room for everybody:
+    injected = the free slots exactly, kept electrons = the first `free` of the unlimited run bit for bit,
+    injected + dropped = the unlimited run's emitters."""
+    Nc, n_i, n_e = 64, 30000, 7900
+    xi = np.where(np.arange(n_i) % 3 == 0, 0.5, Nc - 0.5).astype(np.float32)
+    vi = np.where(np.arange(n_i) % 3 == 0, -1.0, 1.0).astype(np.float32)   # every ion hits a wall
+    xe = (np.arange(n_e, dtype=np.float32) % 60 + 2.25).astype(np.float32)  # electrons at rest, away from the walls
+    ze = np.zeros(n_e, np.float32)
+    res = {}
+    for name, cap_e in (("room", 16384), ("full", 8192)):
+        p = params(2, n_cells=Nc, ppc=1, mcc=False, gamma=0.1, capacity_factor=600)
+        p["species"][0]["capacity"] = cap_e
+        for s in range(2):
+            p["species"][s]["kappa"] = 0.0
+        o = O.Oracle(p)
+        load(o, [(xe, ze, ze, ze), (xi, vi, 0 * xi, 0 * xi)])
+        o.set_E32(np.zeros(Nc + 1, np.float32))
+        rc = o.step(1)
+        m = o.moments(0)
+        # the secondaries go through the step's sort with the survivors; no resting electron sits in the two wall
+        # cells, so the left-wall secondaries are cell 0 and the right-wall ones cell N_c - 1, each in emission
+        # order (the sort is stable).  The ions of cell 0 precede those of cell N_c - 1 in the absorbed list.
+        arr = [o.debug_get(w) for w in (O.X, O.VX, O.VY, O.VZ)]
+        lft, rgt = arr[0] < 1.0, arr[0] >= Nc - 1.0
+        res[name] = (rc, m, [a[lft] for a in arr], int(rgt.sum()))
+        assert m["count"] == n_e + m["injected"] and lft.sum() + rgt.sum() == m["injected"]
+    (rc_r, m_r, l_r, nr_r), (rc_f, m_f, l_f, nr_f) = res["room"], res["full"]
+    free = 8192 - n_e
+    assert rc_r == 0 and m_r["dropped"] == 0 and l_r[0].shape[0] > 2 * free and nr_r > 2 * free
+    assert rc_f == -2 and m_f["injected"] == free and m_f["dropped"] == m_r["injected"] - free
+    assert nr_f == 0                       # the free slots went to the FIRST emitters: all at the left wall
+    for a, b in zip(l_r, l_f):
+        assert np.array_equal(a[:free], b)
+
+
 def test_periodic_clamp_faster_than_a_box_length_and_nan():
     """DESIGN.md R21 (L41 says only "removed"/"inserted" for bounded runs; periodic comes from
     BASELINE.json): ONE wrap is applied per step; a particle that is still outside [0, N_c)
