@@ -89,21 +89,34 @@ def run_oracle_sample(p_full, steps, warmup, full_size=True):
         p = W.make_params(p_full["cfg_id"], n_cells=p_full["n_cells"], ppc=max(8, min(p_full["ppc"], 100)),
                           sort_ratio=p_full["sort_ratio"], courant=p_full["courant"])
     parts = W.make_particles(p)
-    o = O.Oracle(p)
-    for s, a in enumerate(parts):
-        o.load_particles(s, *a)
-    del parts
-    if warmup:
-        o.step(warmup)
-    n0 = sum(o.moments(s)["count"] for s in range(p["n_species"]))
-    t0 = time.perf_counter()
-    o.step(steps)
-    dt = time.perf_counter() - t0
-    n1 = sum(o.moments(s)["count"] for s in range(p["n_species"]))
-    o.close()
+    # the oracle is one thread: pin it to one core for the timed part (BASELINE.md's plan), and say which
+    core, allowed = None, None
+    try:
+        allowed = os.sched_getaffinity(0)
+        core = max(allowed)
+        os.sched_setaffinity(0, {core})
+    except (AttributeError, OSError):
+        core = None
+    try:
+        o = O.Oracle(p)
+        for s, a in enumerate(parts):
+            o.load_particles(s, *a)
+        del parts
+        if warmup:
+            o.step(warmup)
+        n0 = sum(o.moments(s)["count"] for s in range(p["n_species"]))
+        t0 = time.perf_counter()
+        o.step(steps)
+        dt = time.perf_counter() - t0
+        n1 = sum(o.moments(s)["count"] for s in range(p["n_species"]))
+        o.close()
+    finally:
+        if core is not None:
+            os.sched_setaffinity(0, allowed)
     value = 0.5 * (n0 + n1) * steps / dt
-    sample = "%s at ppc=%d (%d particles; the timed GPU workload has ppc=%d), steps %d..%d of the run, oracle single-threaded" % (
-        p["name"], p["ppc"], n0, p_full["ppc"], warmup, warmup + steps)
+    sample = "%s at ppc=%d (%d particles; the timed GPU workload has ppc=%d), steps %d..%d of the run, oracle single-threaded, %s" % (
+        p["name"], p["ppc"], n0, p_full["ppc"], warmup, warmup + steps,
+        "pinned to core %d" % core if core is not None else "not pinned (no sched_setaffinity)")
     return value, dt / steps * 1e3, sample, p["ppc"] == p_full["ppc"]
 
 
@@ -124,12 +137,16 @@ def reference_arm(args, p):
     if rank != 0:
         return
     steps = max(1, min(args.steps, 6 if p["n_per_species"] > 10_000_000 else 50))
-    value, ms, sample, same = run_oracle_sample(p, steps, min(args.warmup, 1))
+    warm = min(args.warmup, 1)
+    value, ms, sample, same = run_oracle_sample(p, steps, warm)
+    # "steps" / "warmup" are the counts actually run (ms_per_step x steps is the timed region); the request, when
+    # it was capped to keep the run within minutes, is kept beside them
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "steps": steps, "warmup": warm, "ms_per_step": ms, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(p), "timed": sample, "timed_steps": steps},
+        "config": {"workload": workload_name(p), "timed": sample, "timed_steps": steps,
+                   "requested_steps": args.steps, "requested_warmup": args.warmup},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
                          "same_config": same, "host_cpu": cpu_model(), "nproc": os.cpu_count()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -406,21 +423,48 @@ def main():
     if args.config == 4 and not args.no_200 and world == 1:
         for s_, sp in enumerate(pinned):
             sim.load_particles(s_, *[t_.numpy() for t_ in sp])
-        tot_ms, tot_ps, chunk = 0.0, 0.0, 10
+        tot_ms, tot_ps, tot_steps = 0.0, 0.0, 0
         c0 = sum(m["count"] for m in live())
-        for _ in range(200 // chunk):
+        hot_ms, hot_ps, hot_k = 0.0, 0.0, None
+        # 8 chunks of 10 (steps 0..80), 3 steps with per-kernel events (80..83, not in the average), 7, 11 x 10
+        for chunk in [10] * 8 + ["kernels"] + [7] + [10] * 11:
+            if chunk == "kernels":      # the dominant kernel in the hot regime, like `roofline` above
+                hk0, t_dom = live(), 0.0
+                for _ in range(3):
+                    for name, s_, kms in sim.step_timed():
+                        if (name, s_) == (dom["kernel"], dom["species"]):
+                            t_dom += kms / 3
+                hk1 = live()
+                c0 = sum(m["count"] for m in hk1)
+                q = dom["species"]
+                hb = algorithmic_bytes(dom["kernel"], 0.5 * (hk0[q]["count"] + hk1[q]["count"]),
+                                       0.5 * (hk0[q]["n_sorted"] + hk1[q]["n_sorted"]), 0, 0, folded[q])
+                hot_k = {"kernel": dom_name, "kernel_ms": t_dom, "alg_bytes_per_launch": hb,
+                         "achieved": hb / (t_dom * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": hb / (t_dom * 1e-3) / 1e9 / peak, "kernel_window": "steps 80..83"}
+                continue
             barrier()
             e0.record(sim.stream)
             sim.step(chunk)
             e1.record(sim.stream)
             barrier()
-            tot_ms += e0.elapsed_time(e1)
+            cms = e0.elapsed_time(e1)
             c1 = sum(m["count"] for m in live())
+            if 60 <= tot_steps < 80:
+                hot_ms += cms
+                hot_ps += 0.5 * (c0 + c1) * chunk
+            tot_ms += cms
             tot_ps += 0.5 * (c0 + c1) * chunk
+            tot_steps += chunk
             c0 = c1
-        run200 = {"value_200": tot_ps / (tot_ms * 1e-3), "ms_per_step_200": tot_ms / 200.0, "unit": UNIT,
-                  "window": "steps 0..200 after a fresh load (config 4's own run), timed in 20 chunks of 10 steps",
-                  "particles_first_last": [2 * p["n_per_species"], c1]}
+        run200 = {"value_200": tot_ps / (tot_ms * 1e-3), "ms_per_step_200": tot_ms / tot_steps, "unit": UNIT,
+                  "window": "steps 0..200 after a fresh load (config 4's own run), timed in chunks of 10 steps; "
+                            "steps 80..83 carry per-kernel events and are left out of the average (%d timed steps)" % tot_steps,
+                  "particles_first_last": [2 * p["n_per_species"], c1],
+                  # the hot regime (electrons heated, windows of the sort wider): the same two figures as the
+                  # headline and as `roofline`, driver-visible instead of a note in profiles/
+                  "hot": dict({"window": "steps 60..80 of the same run", "value": hot_ps / (hot_ms * 1e-3),
+                               "ms_per_step": hot_ms / 20.0}, **(hot_k or {}))}
 
     # end to end through the public API with HOST buffers: every step re-loads the particles from
     # pinned host memory (H2D), advances one step, and reads rho/phi/E back (D2H)

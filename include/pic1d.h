@@ -27,6 +27,13 @@ extern "C" {
 
 #define PIC1D_MAX_SPECIES 2
 
+/* Version of this boundary: bumped whenever a struct layout, a flag, an error code or an entry point changes.
+ * 3 = round 3 (pic1d_graph_launch_count, pic1d_abi_version, validation of e_reflect / coul_A; the names
+ * PIC1D_FLAG_VERIFY_ORDER and PIC1D_ERR_ORDER below are retired -- kept so that callers written against
+ * version 2 still compile; the library ignores the flag and never returns the code).  pic1d_abi_version()
+ * returns the value the loaded library was built with: compare it with this macro after dlopen. */
+#define PIC1D_ABI_VERSION 3
+
 #define PIC1D_OK 0
 #define PIC1D_ERR_ARG (-1)       /* bad argument / bad struct_size / call order */
 #define PIC1D_ERR_CAPACITY (-2)  /* sticky: a load, a birth or an injection exceeded a capacity;   \
@@ -177,6 +184,7 @@ int pic1d_moments(pic1d_t* h, int species, pic1d_moments_t* out, double* density
 int pic1d_destroy(pic1d_t* h);
 
 /* ---- helpers outside the six-call contract ------------------------------------------------- */
+int pic1d_abi_version(void); /* PIC1D_ABI_VERSION of the library that is loaded */
 int pic1d_n_nodes(const pic1d_t* h);
 int pic1d_n_sort_cells(const pic1d_t* h);
 uint32_t pic1d_step_index(const pic1d_t* h);

@@ -3,9 +3,13 @@
 // One stream-ordered kernel sequence per step, no host round trip (contrast PAPER.md L144):
 //   k_step_begin
 //   per species (ions first, so their wall hits can emit secondaries into the electron source):
-//       k_push_count[_w] -> k_bin_scan -> k_offsets_scan -> k_push_scatter[_w] [-> k_see_emit]
+//       k_push_count[_w] -> k_bin_scan (prefix over tiles per sort cell + the offsets scan, last block done)
+//       -> k_push_scatter[_w] (species with sparse candidates: MCC folded in) [-> k_see_emit after the ions]
 //       (_w: barrier-free warp-tile kernels for species that obey Eq. 5, pic1d_sort_warp.cuh)
-//   k_deposit per species -> k_rho_combine -> k_field -> k_mcc per species
+//   main stream: k_deposit (one launch, every species) -> k_field[_smem] (rho combine + Poisson + E)
+//   side stream, beside them: k_mcc -> k_mcc_births per species with a pass of its own, k_null_bits_next (the
+//       null-test masks of the folded species for the NEXT step), [k_coulomb]
+// 13 launches for config 4; pairs of steps are replayed from a captured CUDA graph (pic1d_step).
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -fmad=false (see ../build.py).
 #include <cmath>
 #include <cstdio>
@@ -791,6 +795,7 @@ int pic1d_n_nodes(const pic1d_t* h) { return h ? h->nodes : PIC1D_ERR_ARG; }
 int pic1d_n_sort_cells(const pic1d_t* h) { return h ? h->n_sc : PIC1D_ERR_ARG; }
 uint32_t pic1d_step_index(const pic1d_t* h) { return h ? h->step : 0u; }
 const char* pic1d_last_cuda_error(const pic1d_t* h) { return h ? cudaGetErrorString(h->last_err) : "null handle"; }
+int pic1d_abi_version(void) { return PIC1D_ABI_VERSION; }
 int64_t pic1d_launch_count(const pic1d_t* h) { return h ? h->launches : 0; }
 int64_t pic1d_graph_launch_count(const pic1d_t* h) { return !h ? 0 : h->graph_off ? -1 : h->graph_launches; }
 

@@ -7,9 +7,9 @@
 //   pass 1  k_push_count    read x, vx (8 B/particle); push; boundary; key; per-tile histogram in
 //                           shared memory; the tile's window [lo, hi] of counts goes to a pool
 //   scan    k_bin_scan      per sort cell k: exclusive prefix over tiles of count[t][k] (in place),
-//                           total -> hist[k]
-//                           (+ one extra block: prefix of the per-tile absorbed counts)
-//           k_offsets_scan  exclusive scan of hist -> offsets[N_sc + 1]
+//                           total -> hist[k]; the last block to finish scans hist -> offsets[N_sc + 1]
+//                           (+ 64 extra blocks: chunked prefix of the per-tile absorbed counts; + blocks that
+//                           compute a folded species' null-test mask when it was not computed one step ahead)
 //   pass 2  k_push_scatter  read x, vx, vy, vz (16 B); identical push; stable rank inside the tile
 //                           (warp-private shared counters, warps in order); write the four arrays to
 //                           offsets[k] + prefix[t][k] + rank (16 B), through a tile-sorted shared-memory

@@ -26,7 +26,9 @@ _DBG_DTYPE = {DBG_X: np.float32, DBG_VX: np.float32, DBG_VY: np.float32, DBG_VZ:
               DBG_KEYS: np.int32, DBG_OFFSETS: np.int32, DBG_MASK: np.uint8, DBG_E32: np.float32,
               DBG_RHO_S: np.float64, DBG_TILE_W: np.int32, DBG_PARTNER: np.int32}
 
-EXPORTS = ["pic1d_workspace_bytes", "pic1d_create", "pic1d_load_particles", "pic1d_step",
+ABI_VERSION = 3   # PIC1D_ABI_VERSION of include/pic1d.h this binding was written against
+
+EXPORTS = ["pic1d_abi_version", "pic1d_workspace_bytes", "pic1d_create", "pic1d_load_particles", "pic1d_step",
            "pic1d_get_rho_phi_E", "pic1d_moments", "pic1d_destroy", "pic1d_n_nodes",
            "pic1d_n_sort_cells", "pic1d_step_index", "pic1d_last_cuda_error", "pic1d_launch_count",
            "pic1d_graph_launch_count", "pic1d_step_timed", "pic1d_debug_count", "pic1d_debug_get", "pic1d_debug_set_E32",
@@ -78,6 +80,10 @@ def load_library():
             raise RuntimeError("CUDA library %s is missing: run `python -m paper_1104_3998_b200.build` "
                                "(there is no CPU fallback)" % LIB_PATH)
         lib = C.CDLL(LIB_PATH)
+        have = lib.pic1d_abi_version() if hasattr(lib, "pic1d_abi_version") else 2
+        if have != ABI_VERSION:     # a stale in-tree build: struct layouts may differ, refuse instead of guessing
+            raise RuntimeError("%s was built for ABI version %d, this binding needs %d: rebuild it with "
+                               "`python -m paper_1104_3998_b200.build`" % (LIB_PATH, have, ABI_VERSION))
         lib.pic1d_last_cuda_error.restype = C.c_char_p
         lib.pic1d_launch_count.restype = C.c_int64
         lib.pic1d_graph_launch_count.restype = C.c_int64
