@@ -40,7 +40,8 @@ def measured_peak():
 def workload_name(p):
     return "config[%d] %s: %d cells x %d ppc x %d species, r=%g%s" % (
         p["cfg_id"], p["name"], p["n_cells"], p["ppc"], p["n_species"], p["sort_ratio"],
-        " (Courant twin)" if p["courant"] else "")
+        " (Courant twin)" if p["courant"] else "") + (
+        " + binary Coulomb collisions in the sort cells" if any(a > 0 for a in p.get("coul_A", [])) else "")
 
 
 # ---------------------------------------------------------------------------------------------
@@ -172,6 +173,8 @@ def algorithmic_bytes(name, n_src, n_out, cand_frac, coll_frac, folded):
     if name == "mcc":
         rd, wr = mcc_bytes_per_particle(cand_frac, coll_frac)
         return (rd + wr) * n_out
+    if name == "coulomb":
+        return 24.0 * n_out                      # every particle has a partner: vx, vy, vz read and written
     return 0.0
 
 
@@ -263,6 +266,8 @@ def main():
     ap.add_argument("--no-graph", action="store_true", help="no CUDA graph replay in pic1d_step")
     ap.add_argument("--mcc-gather", action="store_true", help="k_mcc without the bulk-copy staging of velocities")
     ap.add_argument("--fold-all", action="store_true", help="fold the collisions of every species into its scatter")
+    ap.add_argument("--coulomb", action="store_true",
+                    help="binary Coulomb collisions inside the sort cells on (f3, k_coulomb); off in BASELINE's configs")
     ap.add_argument("--gsort", action="store_true",
                     help="f2: time the paper's gapped in-place push + sort on the ions beside the compact sort")
     ap.add_argument("--profile", action="store_true",
@@ -271,7 +276,7 @@ def main():
     assert args.warmup >= 3 or args.impl == "reference", "timing rule: at least 3 warm-up steps"
 
     p = W.make_params(args.config, n_cells=args.n_cells, ppc=args.ppc, sort_ratio=args.sort_ratio,
-                      courant=args.courant)
+                      courant=args.courant, coulomb=args.coulomb)
     if args.impl == "reference":
         return reference_arm(args, p)
     if args.no_fold:

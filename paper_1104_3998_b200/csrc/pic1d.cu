@@ -320,6 +320,7 @@ int occupancy_grid(pic1d* h, sort_kernel_t kernel, size_t smem) {
 // step's (with the species' MCC folded in, unless PIC1D_FLAG_NO_FOLD)
 void setup_launch(pic1d* h) {
     cudaFuncSetAttribute(k_field_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, FIELD_SMEM_MAX * (int)sizeof(double));
+    cudaFuncSetAttribute(k_coulomb, cudaFuncAttributeMaxDynamicSharedMemorySize, 6144 * 12);
     cudaFuncSetAttribute(k_mcc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     cudaFuncSetAttribute(k_mcc<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * MCC_TILE * sizeof(float)));
     h->WA = std::min((h->n_sc + 1 + 7) / 8 * 8, PIC1D_WA_MAX);
@@ -467,7 +468,10 @@ void enqueue_mcc(pic1d* h, cudaStream_t st) {
         ca.vx = p.buf[p.cur][1]; ca.vy = p.buf[p.cur][2]; ca.vz = p.buf[p.cur][3];
         ca.offsets = p.offsets; ca.partner = p.partner; ca.st = h->st; ca.s = s; ca.n_sc = h->n_sc;
         ca.A = (float)c.coul_A[s]; ca.k0 = (uint32_t)c.seed; ca.k1 = (uint32_t)(c.seed >> 32);
-        k_coulomb<<<std::min(h->n_sc, h->num_sms * 8), PIC1D_NT, 0, st>>>(ca);
+        // staging for cells of up to twice the mean count the arrays were sized for, 72 KB at most (3 blocks / SM)
+        const int64_t per_cell = p.capacity / std::max(1, h->n_sc);
+        ca.slots = (int)std::min<int64_t>(6144, std::max<int64_t>(1024, (2 * per_cell + 255) / 256 * 256));
+        k_coulomb<<<std::min(h->n_sc, h->num_sms * 8), PIC1D_NT, (size_t)ca.slots * 12, st>>>(ca);
         mark(h, "coulomb", s);
     }
 }

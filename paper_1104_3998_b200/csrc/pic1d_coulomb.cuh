@@ -11,7 +11,7 @@
 // rounds on 2h bits (4^h >= n) keyed by philox(cell, step, COUL + s, 0), cycle-walked into [0, n) -- so that any
 // pairing of the cell can come out; pairs (pi(2m), pi(2m+1)); for odd n slot pi(n-1) sits out (not Takizuka-Abe's
 // three-particle rule).  Every thread evaluates pi for its own pairs: integer work, bit-identical to the oracle's.
-// One block per sort cell, one thread per pair; the cell's velocities (12 B x n) are gathered through L1.
+// One block per sort cell, one thread per pair; the cell's velocities (12 B x n) are staged in shared memory.
 // fp32 operations in the order the oracle states them (-fmad=false: nothing is contracted).
 #pragma once
 #include "pic1d_device.cuh"
@@ -25,6 +25,7 @@ struct CoulombArgs {
     int s, n_sc;
     float A;               // coul_A
     uint32_t k0, k1;
+    int slots;             // particles per cell the shared-memory staging holds (dynamic smem = 12 B x slots)
 };
 
 __device__ __forceinline__ unsigned coul_feistel(unsigned m, unsigned n, unsigned h, const uint32_t (&w)[4]) {
@@ -44,7 +45,50 @@ __device__ __forceinline__ unsigned coul_feistel(unsigned m, unsigned n, unsigne
     return x;
 }
 
+// One pair: the oracle's operation order, on values read from / written to `vx, vy, vz` at ia, ib (global arrays
+// with global slots, or the cell's shared-memory copy with slots relative to the cell).  `key` = the pair's first
+// GLOBAL slot (the Philox counter).
+__device__ __forceinline__ void coul_pair(float* vx, float* vy, float* vz, unsigned ia, unsigned ib, unsigned key,
+                                          uint32_t step, uint32_t stream, const CoulombArgs& a, float fn) {
+    const float vxa = vx[ia], vya = vy[ia], vza = vz[ia];
+    const float vxb = vx[ib], vyb = vy[ib], vzb = vz[ib];
+    const float ux = vxa - vxb, uy = vya - vyb, uz = vza - vzb;
+    const float up2 = ux * ux + uy * uy;
+    const float u2 = up2 + uz * uz;
+    if (!(u2 > 0.0f)) return;
+    uint32_t r[4];
+    philox4x32_10(key, step, stream, 1u, a.k0, a.k1, r);  // keyed on the pair's first slot
+    const float uu = sqrtf(u2), up = sqrtf(up2);
+    const float var = (a.A * fn) / (u2 * uu);
+    const float delta = sqrtf(var) * (bm_r(u01(r[0])) * cosf(6.2831855f * u01(r[1])));
+    const float d2 = delta * delta;
+    const float sint = (2.0f * delta) / (1.0f + d2);
+    const float omc = (2.0f * d2) / (1.0f + d2);  // 1 - cos(theta)
+    const float ph = 6.2831855f * u01(r[2]);
+    const float cp = cosf(ph), sp = sinf(ph);
+    float dux, duy, duz;
+    if (up > 0.0f) {
+        dux = ((ux / up) * uz) * (sint * cp) - ((uy / up) * uu) * (sint * sp) - ux * omc;
+        duy = ((uy / up) * uz) * (sint * cp) + ((ux / up) * uu) * (sint * sp) - uy * omc;
+        duz = -(up * (sint * cp)) - uz * omc;
+    } else {
+        dux = uu * (sint * cp); duy = uu * (sint * sp); duz = -(uz * omc);
+    }
+    vx[ia] = vxa + 0.5f * dux; vy[ia] = vya + 0.5f * duy; vz[ia] = vza + 0.5f * duz;
+    vx[ib] = vxb - 0.5f * dux; vy[ib] = vyb - 0.5f * duy; vz[ib] = vzb - 0.5f * duz;
+}
+
+// A cell of up to a.slots particles is staged: its three velocity arrays are read into shared memory with
+// coalesced loads, the pairs (random slots of the cell) are scattered there, and the arrays are written back
+// coalesced -- the partners' gathers cost shared-memory bank conflicts instead of one 32-byte sector per lane
+// (measured on config 4: 29.6 sectors per request, 0.09 of the HBM peak before; profiles/r3_next_kernels.md).
+// Larger cells take the gathered path.  Every particle is in at most one pair, so the order of the pairs does not
+// matter and both paths give the bits of the oracle's sequential loop.
 __global__ void __launch_bounds__(PIC1D_NT) k_coulomb(CoulombArgs a) {
+    extern __shared__ float s_v[];  // [3 * a.slots]
+    float* const s_vx = s_v;
+    float* const s_vy = s_v + a.slots;
+    float* const s_vz = s_v + 2 * a.slots;
     const int tid = threadIdx.x, lane = tid & 31;
     const uint32_t step = a.st->step;
     const uint32_t stream = STREAM_COUL + (uint32_t)a.s;
@@ -61,37 +105,26 @@ __global__ void __launch_bounds__(PIC1D_NT) k_coulomb(CoulombArgs a) {
         while ((1ull << (2u * h)) < n) ++h;  // 4^h >= n
         const float fn = (float)n;
         if (a.partner && (n & 1u) && tid == 0) a.partner[off + coul_feistel(n - 1u, n, h, w)] = -1;
-        for (unsigned m = 2u * tid; m + 1u < n; m += 2u * PIC1D_NT) {
-            const unsigned ia = off + coul_feistel(m, n, h, w);
-            const unsigned ib = off + coul_feistel(m + 1u, n, h, w);
-            if (a.partner) { a.partner[ia] = (int)ib; a.partner[ib] = (int)ia; }
-            ++n_pairs;
-            const float vxa = a.vx[ia], vya = a.vy[ia], vza = a.vz[ia];
-            const float vxb = a.vx[ib], vyb = a.vy[ib], vzb = a.vz[ib];
-            const float ux = vxa - vxb, uy = vya - vyb, uz = vza - vzb;
-            const float up2 = ux * ux + uy * uy;
-            const float u2 = up2 + uz * uz;
-            if (!(u2 > 0.0f)) continue;
-            uint32_t r[4];
-            philox4x32_10(ia, step, stream, 1u, a.k0, a.k1, r);  // keyed on the pair's first slot
-            const float uu = sqrtf(u2), up = sqrtf(up2);
-            const float var = (a.A * fn) / (u2 * uu);
-            const float delta = sqrtf(var) * (bm_r(u01(r[0])) * cosf(6.2831855f * u01(r[1])));
-            const float d2 = delta * delta;
-            const float sint = (2.0f * delta) / (1.0f + d2);
-            const float omc = (2.0f * d2) / (1.0f + d2);  // 1 - cos(theta)
-            const float ph = 6.2831855f * u01(r[2]);
-            const float cp = cosf(ph), sp = sinf(ph);
-            float dux, duy, duz;
-            if (up > 0.0f) {
-                dux = ((ux / up) * uz) * (sint * cp) - ((uy / up) * uu) * (sint * sp) - ux * omc;
-                duy = ((uy / up) * uz) * (sint * cp) + ((ux / up) * uu) * (sint * sp) - uy * omc;
-                duz = -(up * (sint * cp)) - uz * omc;
-            } else {
-                dux = uu * (sint * cp); duy = uu * (sint * sp); duz = -(uz * omc);
+        const bool staged = n <= (unsigned)a.slots;  // block-uniform
+        if (staged) {
+            for (unsigned i = tid; i < n; i += PIC1D_NT) {
+                s_vx[i] = a.vx[off + i]; s_vy[i] = a.vy[off + i]; s_vz[i] = a.vz[off + i];
             }
-            a.vx[ia] = vxa + 0.5f * dux; a.vy[ia] = vya + 0.5f * duy; a.vz[ia] = vza + 0.5f * duz;
-            a.vx[ib] = vxb - 0.5f * dux; a.vy[ib] = vyb - 0.5f * duy; a.vz[ib] = vzb - 0.5f * duz;
+            __syncthreads();
+        }
+        for (unsigned m = 2u * tid; m + 1u < n; m += 2u * PIC1D_NT) {
+            const unsigned ia = coul_feistel(m, n, h, w), ib = coul_feistel(m + 1u, n, h, w);
+            if (a.partner) { a.partner[off + ia] = (int)(off + ib); a.partner[off + ib] = (int)(off + ia); }
+            ++n_pairs;
+            if (staged) coul_pair(s_vx, s_vy, s_vz, ia, ib, off + ia, step, stream, a, fn);
+            else coul_pair(a.vx, a.vy, a.vz, off + ia, off + ib, off + ia, step, stream, a, fn);
+        }
+        if (staged) {
+            __syncthreads();
+            for (unsigned i = tid; i < n; i += PIC1D_NT) {
+                a.vx[off + i] = s_vx[i]; a.vy[off + i] = s_vy[i]; a.vz[off + i] = s_vz[i];
+            }
+            __syncthreads();  // the next cell overwrites the staging arrays
         }
     }
     n_pairs = __reduce_add_sync(0xffffffffu, n_pairs);
